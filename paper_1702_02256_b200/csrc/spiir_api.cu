@@ -1,0 +1,344 @@
+// spiir_api.cu -- C ABI of libspiir.so: plans, launches, resamplers, multirate composition.
+// See include/spiir.h for the contract of every entry point.
+#include <stdio.h>
+#include <string.h>
+
+#include <algorithm>
+#include <new>
+#include <vector>
+
+#include "spiir_filter.cuh"
+#include "spiir_internal.h"
+#include "spiir_resample.cuh"
+
+namespace spiir {
+
+spiir_status cuda_fail(cudaError_t e, const char* what)
+{
+    set_error("CUDA error %d (%s) in %s", (int)e, cudaGetErrorString(e), what);
+    return e == cudaErrorMemoryAllocation ? SPIIR_ENOMEM : SPIIR_ECUDA;
+}
+
+spiir_status device_info(DeviceInfo* out)
+{
+    int dev = 0;
+    SPIIR_CUDA(cudaGetDevice(&dev));
+    out->device = dev;
+    SPIIR_CUDA(cudaDeviceGetAttribute(&out->n_sm, cudaDevAttrMultiProcessorCount, dev));
+    SPIIR_CUDA(cudaDeviceGetAttribute(&out->smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
+    return SPIIR_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+// kernel dispatch table: (F, LPT, NOZ) -> instantiation
+// ---------------------------------------------------------------------------------------------
+typedef void (*filter_kernel_t)(const FilterArgs);
+
+template <int F, int LPT>
+static filter_kernel_t pick_noz(bool noz)
+{
+    return noz ? (filter_kernel_t)spiir_filter_kernel<F, LPT, true> : (filter_kernel_t)spiir_filter_kernel<F, LPT, false>;
+}
+
+template <int LPT>
+static filter_kernel_t pick_small(int F, bool noz)
+{
+    switch (F) {
+        case 1: return pick_noz<1, LPT>(noz);
+        case 2: return pick_noz<2, LPT>(noz);
+        case 3: return pick_noz<3, LPT>(noz);
+        case 4: return pick_noz<4, LPT>(noz);
+    }
+    return nullptr;
+}
+
+static filter_kernel_t pick_kernel(int F, int LPT, bool noz)
+{
+    switch (LPT) {
+        case 1: return pick_small<1>(F, noz);
+        case 2: return pick_small<2>(F, noz);
+        case 4: return pick_small<4>(F, noz);
+        case 8: return pick_small<8>(F, noz);
+        case 32:
+            switch (F) {
+                case 1: return pick_noz<1, 32>(noz);
+                case 2: return pick_noz<2, 32>(noz);
+                case 3: return pick_noz<3, 32>(noz);
+                case 4: return pick_noz<4, 32>(noz);
+                case 5: return pick_noz<5, 32>(noz);
+                case 6: return pick_noz<6, 32>(noz);
+                case 7: return pick_noz<7, 32>(noz);
+                case 8: return pick_noz<8, 32>(noz);
+                case 10: return pick_noz<10, 32>(noz);
+                case 12: return pick_noz<12, 32>(noz);
+                case 14: return pick_noz<14, 32>(noz);
+                case 16: return pick_noz<16, 32>(noz);
+            }
+    }
+    return nullptr;
+}
+
+spiir_status plan_geometry(const spiir_plan* p, int n, FilterGeometry* g)
+{
+    return compute_geometry(p->T, p->L, p->S, p->Dpad, n, p->opt_chunks, p->NC_cap, p->dev.n_sm, p->dev.smem_optin, g);
+}
+
+spiir_status filter_launch(spiir_plan* p, const float* x, int n, spiir_c64* z, int accumulate, cudaStream_t st)
+{
+    FilterGeometry g;
+    spiir_status rc = plan_geometry(p, n, &g);
+    if (rc != SPIIR_OK) return rc;
+    FilterArgs a;
+    a.coef = p->d_coef; a.dly = p->d_dly; a.state = p->d_state; a.chunk_st = p->d_chunk;
+    a.hist = p->d_hist[p->hist_cur]; a.hist_next = p->d_hist[p->hist_cur ^ 1];
+    a.x = x; a.z = reinterpret_cast<float2*>(z);
+    a.n = n; a.T = p->T; a.G = p->G; a.S = p->S; a.Dpad = p->Dpad;
+    a.NT = g.NT; a.CS = g.CS; a.NC = g.NC; a.C = g.C;
+    a.x_aligned = ((reinterpret_cast<uintptr_t>(x) & 15u) == 0 && (p->S == 1 || (n & 3) == 0)) ? 1 : 0;
+    a.accumulate = accumulate;
+    const dim3 grid(g.grid_x, g.grid_y), block(g.warps * 32);
+    for (int pass = 0; pass < (g.NC > 1 ? 2 : 1); ++pass) {
+        a.mode = g.NC > 1 ? pass + 1 : 0;
+        filter_kernel_t k = pick_kernel(g.F, g.LPT, a.mode == 1);
+        if (!k) { set_error("no kernel for F=%d LPT=%d", g.F, g.LPT); return SPIIR_EUNSUPPORTED; }
+        SPIIR_CUDA(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, g.smem_bytes));
+        k<<<grid, block, g.smem_bytes, st>>>(a);
+        SPIIR_CUDA(cudaGetLastError());
+        if (a.mode == 1) {
+            const int nf = (int)p->nfilt;
+            spiir_chunk_carry_kernel<<<(nf + 255) / 256, 256, 0, st>>>(p->d_coef, p->d_state, p->d_chunk, nf, p->S, g.NC, g.C);
+            SPIIR_CUDA(cudaGetLastError());
+        }
+    }
+    p->hist_cur ^= 1;
+    return SPIIR_OK;
+}
+
+}  // namespace spiir
+
+using namespace spiir;
+
+extern "C" {
+
+void spiir_plan_destroy(spiir_plan_t* p)
+{
+    if (!p) return;
+    cudaFree(p->d_coef); cudaFree(p->d_dly); cudaFree(p->d_state); cudaFree(p->d_chunk);
+    cudaFree(p->d_hist[0]); cudaFree(p->d_hist[1]); cudaFree(p->d_pos);
+    delete p;
+}
+
+spiir_status spiir_plan_create(spiir_plan_t** out, const spiir_c64* a1, const spiir_c64* b0, const int32_t* delays,
+                               int n_templates, int n_filters, int rate_hz, const spiir_plan_opts* opts)
+{
+    if (!out) { set_error("spiir_plan_create: out is NULL"); return SPIIR_EINVAL; }
+    *out = nullptr;
+    if (!a1 || !b0 || !delays || n_templates < 1 || n_filters < 1) {
+        set_error("spiir_plan_create: NULL array or non-positive shape");
+        return SPIIR_EINVAL;
+    }
+    spiir_plan_opts o = {1, 4096, 0, 0};
+    if (opts) o = *opts;
+    if (o.n_streams < 1 || o.max_block < 1 || o.time_chunks < 0) {
+        set_error("spiir_plan_create: bad options");
+        return SPIIR_EINVAL;
+    }
+    const size_t TL = (size_t)n_templates * n_filters;
+    int dmax = 0;
+    for (size_t i = 0; i < TL; ++i) {
+        if (delays[i] < 0 || delays[i] >= (1 << 20)) { set_error("spiir_plan_create: delay out of range at %zu", i); return SPIIR_EINVAL; }
+        dmax = std::max(dmax, (int)delays[i]);
+    }
+    int F, LPT;
+    if (!choose_lane_mapping(n_filters, &F, &LPT)) {
+        set_error("spiir_plan_create: n_filters = %d not supported (1..512)", n_filters);
+        return SPIIR_EUNSUPPORTED;
+    }
+    spiir_plan* p = new (std::nothrow) spiir_plan;
+    if (!p) return SPIIR_ENOMEM;
+    spiir_status rc = device_info(&p->dev);
+    if (rc != SPIIR_OK) { delete p; return rc; }
+    p->T = n_templates; p->L = n_filters; p->S = o.n_streams; p->rate_hz = rate_hz; p->max_block = o.max_block;
+    p->Dmax = dmax; p->Dpad = std::max(4, (dmax + 3) / 4 * 4);
+    p->F = F; p->LPT = LPT; p->TPG = 32 / LPT; p->G = (n_templates + p->TPG - 1) / p->TPG;
+    p->nfilt = (size_t)p->G * F * 32;
+    p->opt_chunks = o.time_chunks; p->flags = o.flags;
+    // chunk scratch: sized for the geometry of the largest block, at most 256 MiB
+    p->NC_cap = 1 << 20;
+    FilterGeometry g;
+    rc = plan_geometry(p, o.max_block, &g);
+    if (rc != SPIIR_OK) { delete p; return rc; }
+    int nc = g.NC;
+    while (nc > 1 && (size_t)nc * p->S * p->nfilt * sizeof(float2) > ((size_t)256 << 20)) nc /= 2;
+    p->NC_cap = std::max(1, nc);
+
+    std::vector<float> coef;
+    std::vector<int32_t> dly, pos;
+    build_layout(a1, b0, delays, n_templates, n_filters, F, LPT, (o.flags & 1) == 0, &coef, &dly, &pos);
+    p->conflict_degree = layout_conflict_degree(dly, p->G, F);
+
+#define SPIIR_TRY(call)                                                                 \
+    do {                                                                                \
+        cudaError_t e__ = (call);                                                       \
+        if (e__ != cudaSuccess) { spiir_status s__ = cuda_fail(e__, #call); spiir_plan_destroy(p); return s__; } \
+    } while (0)
+    SPIIR_TRY(cudaMalloc(&p->d_coef, p->nfilt * sizeof(float4)));
+    SPIIR_TRY(cudaMalloc(&p->d_dly, p->nfilt * sizeof(int32_t)));
+    SPIIR_TRY(cudaMalloc(&p->d_state, (size_t)p->S * p->nfilt * sizeof(float2)));
+    SPIIR_TRY(cudaMalloc(&p->d_pos, TL * sizeof(int32_t)));
+    SPIIR_TRY(cudaMalloc(&p->d_hist[0], (size_t)p->S * p->Dpad * sizeof(float)));
+    SPIIR_TRY(cudaMalloc(&p->d_hist[1], (size_t)p->S * p->Dpad * sizeof(float)));
+    if (p->NC_cap > 1) SPIIR_TRY(cudaMalloc(&p->d_chunk, (size_t)p->NC_cap * p->S * p->nfilt * sizeof(float2)));
+    SPIIR_TRY(cudaMemcpy(p->d_coef, coef.data(), p->nfilt * sizeof(float4), cudaMemcpyHostToDevice));
+    SPIIR_TRY(cudaMemcpy(p->d_dly, dly.data(), p->nfilt * sizeof(int32_t), cudaMemcpyHostToDevice));
+    SPIIR_TRY(cudaMemcpy(p->d_pos, pos.data(), TL * sizeof(int32_t), cudaMemcpyHostToDevice));
+    SPIIR_TRY(cudaMemset(p->d_state, 0, (size_t)p->S * p->nfilt * sizeof(float2)));
+    SPIIR_TRY(cudaMemset(p->d_hist[0], 0, (size_t)p->S * p->Dpad * sizeof(float)));
+    SPIIR_TRY(cudaMemset(p->d_hist[1], 0, (size_t)p->S * p->Dpad * sizeof(float)));
+    if (p->d_chunk) SPIIR_TRY(cudaMemset(p->d_chunk, 0, (size_t)p->NC_cap * p->S * p->nfilt * sizeof(float2)));
+#undef SPIIR_TRY
+    *out = p;
+    return SPIIR_OK;
+}
+
+spiir_status spiir_filter(spiir_plan_t* p, const float* x, int n, spiir_c64* snr_out, void* cuda_stream)
+{
+    if (!p || n < 0) { set_error("spiir_filter: bad plan or n"); return SPIIR_EINVAL; }
+    if (n == 0) return SPIIR_OK;
+    if (!x || !snr_out) { set_error("spiir_filter: NULL buffer"); return SPIIR_EINVAL; }
+    if (n > p->max_block) { set_error("spiir_filter: n = %d exceeds max_block = %d", n, p->max_block); return SPIIR_ESTATE; }
+    if (reinterpret_cast<uintptr_t>(x) & 3u || reinterpret_cast<uintptr_t>(snr_out) & 7u) {
+        set_error("spiir_filter: x must be 4-byte and snr_out 8-byte aligned");
+        return SPIIR_EINVAL;
+    }
+    return filter_launch(p, x, n, snr_out, 0, static_cast<cudaStream_t>(cuda_stream));
+}
+
+spiir_status spiir_plan_reset(spiir_plan_t* p, void* cuda_stream)
+{
+    if (!p) { set_error("spiir_plan_reset: NULL plan"); return SPIIR_EINVAL; }
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    SPIIR_CUDA(cudaMemsetAsync(p->d_state, 0, (size_t)p->S * p->nfilt * sizeof(float2), st));
+    SPIIR_CUDA(cudaMemsetAsync(p->d_hist[0], 0, (size_t)p->S * p->Dpad * sizeof(float), st));
+    SPIIR_CUDA(cudaMemsetAsync(p->d_hist[1], 0, (size_t)p->S * p->Dpad * sizeof(float), st));
+    return SPIIR_OK;
+}
+
+spiir_status spiir_plan_launch_info(const spiir_plan_t* p, int n, int info[8])
+{
+    if (!p || !info || n < 1) { set_error("spiir_plan_launch_info: bad arguments"); return SPIIR_EINVAL; }
+    FilterGeometry g;
+    spiir_status rc = plan_geometry(p, n, &g);
+    if (rc != SPIIR_OK) return rc;
+    info[0] = g.F; info[1] = g.LPT; info[2] = g.warps; info[3] = g.grid_x * g.grid_y;
+    info[4] = g.NC; info[5] = g.smem_bytes; info[6] = g.NT; info[7] = g.launches;
+    return SPIIR_OK;
+}
+
+static spiir_status state_permute(spiir_plan_t* p, spiir_c64* user, int to_user, void* cuda_stream)
+{
+    if (!p || !user) { set_error("spiir_plan_get/set_state: NULL argument"); return SPIIR_EINVAL; }
+    const int TL = p->T * p->L;
+    spiir_state_permute_kernel<<<(TL + 255) / 256, 256, 0, static_cast<cudaStream_t>(cuda_stream)>>>(
+        p->d_state, reinterpret_cast<float2*>(user), p->d_pos, TL, (int)p->nfilt, p->S, to_user);
+    SPIIR_CUDA(cudaGetLastError());
+    return SPIIR_OK;
+}
+spiir_status spiir_plan_get_state(spiir_plan_t* p, spiir_c64* y_out, void* cuda_stream) { return state_permute(p, y_out, 1, cuda_stream); }
+spiir_status spiir_plan_set_state(spiir_plan_t* p, const spiir_c64* y_in, void* cuda_stream)
+{
+    return state_permute(p, const_cast<spiir_c64*>(y_in), 0, cuda_stream);
+}
+
+// ---------------------------------------------------------------------------------------------
+// Resamplers
+// ---------------------------------------------------------------------------------------------
+void spiir_resamp_destroy(spiir_resamp_t* r)
+{
+    if (!r) return;
+    cudaFree(r->d_taps); cudaFree(r->d_hist[0]); cudaFree(r->d_hist[1]);
+    delete r;
+}
+
+spiir_status spiir_resamp_create(spiir_resamp_t** out, int direction, int n_taps, double kaiser_beta, double cutoff,
+                                 int n_rows, int max_block)
+{
+    if (!out) { set_error("spiir_resamp_create: out is NULL"); return SPIIR_EINVAL; }
+    *out = nullptr;
+    if ((direction != SPIIR_DOWN2 && direction != SPIIR_UP2) || n_taps < 2 || n_taps > kMaxTaps || (n_taps & 1) ||
+        n_rows < 1 || max_block < 1) {
+        set_error("spiir_resamp_create: bad arguments");
+        return SPIIR_EINVAL;
+    }
+    spiir_resamp* r = new (std::nothrow) spiir_resamp;
+    if (!r) return SPIIR_ENOMEM;
+    r->taps.resize(n_taps);
+    spiir_status rc = kaiser_taps(n_taps, kaiser_beta, cutoff, r->taps.data());
+    if (rc == SPIIR_OK) rc = device_info(&r->dev);
+    if (rc != SPIIR_OK) { delete r; return rc; }
+    r->direction = direction; r->N = n_taps; r->rows = n_rows; r->max_block = max_block;
+    r->H = direction == SPIIR_DOWN2 ? n_taps - 1 : n_taps / 2 - 1;
+    const size_t hbytes = (size_t)n_rows * std::max(1, r->H) * (direction == SPIIR_DOWN2 ? sizeof(float) : sizeof(float2));
+    cudaError_t e = cudaMalloc(&r->d_taps, n_taps * sizeof(float));
+    if (e == cudaSuccess) e = cudaMalloc(&r->d_hist[0], hbytes);
+    if (e == cudaSuccess) e = cudaMalloc(&r->d_hist[1], hbytes);
+    if (e == cudaSuccess) e = cudaMemcpy(r->d_taps, r->taps.data(), n_taps * sizeof(float), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemset(r->d_hist[0], 0, hbytes);
+    if (e == cudaSuccess) e = cudaMemset(r->d_hist[1], 0, hbytes);
+    if (e != cudaSuccess) { rc = cuda_fail(e, "spiir_resamp_create allocation"); spiir_resamp_destroy(r); return rc; }
+    *out = r;
+    return SPIIR_OK;
+}
+
+spiir_status spiir_resamp_reset(spiir_resamp_t* r, void* cuda_stream)
+{
+    if (!r) { set_error("spiir_resamp_reset: NULL"); return SPIIR_EINVAL; }
+    const size_t hbytes = (size_t)r->rows * std::max(1, r->H) * (r->direction == SPIIR_DOWN2 ? sizeof(float) : sizeof(float2));
+    SPIIR_CUDA(cudaMemsetAsync(r->d_hist[0], 0, hbytes, static_cast<cudaStream_t>(cuda_stream)));
+    SPIIR_CUDA(cudaMemsetAsync(r->d_hist[1], 0, hbytes, static_cast<cudaStream_t>(cuda_stream)));
+    return SPIIR_OK;
+}
+
+spiir_status spiir_resample_down(spiir_resamp_t* r, const float* in, int n_in, float* out, void* cuda_stream)
+{
+    if (!r || r->direction != SPIIR_DOWN2 || n_in < 0 || (n_in & 1)) { set_error("spiir_resample_down: bad plan or odd n_in"); return SPIIR_EINVAL; }
+    if (n_in == 0) return SPIIR_OK;
+    if (!in || !out) { set_error("spiir_resample_down: NULL buffer"); return SPIIR_EINVAL; }
+    if (n_in > r->max_block) { set_error("spiir_resample_down: n_in exceeds max_block"); return SPIIR_ESTATE; }
+    ResampArgs a;
+    a.taps = r->d_taps; a.in = in; a.out = out; a.hist = r->d_hist[r->hist_cur]; a.hist_next = r->d_hist[r->hist_cur ^ 1];
+    a.rows = r->rows; a.n_in = n_in; a.N = r->N; a.accumulate = 0;
+    const int n_out = n_in / 2;
+    a.tile = std::min(512, (n_out + 127) / 128 * 128);
+    const dim3 grid(r->rows, (n_out + a.tile - 1) / a.tile);
+    const size_t smem = (size_t)(r->N + 2 * (a.tile + r->N / 2)) * sizeof(float);
+    spiir_down2_kernel<<<grid, 128, smem, static_cast<cudaStream_t>(cuda_stream)>>>(a);
+    SPIIR_CUDA(cudaGetLastError());
+    r->hist_cur ^= 1;
+    return SPIIR_OK;
+}
+
+spiir_status spiir_resample_up(spiir_resamp_t* r, const spiir_c64* in, int n_in, spiir_c64* out, int accumulate,
+                               void* cuda_stream)
+{
+    if (!r || r->direction != SPIIR_UP2 || n_in < 0) { set_error("spiir_resample_up: bad plan or n_in"); return SPIIR_EINVAL; }
+    if (n_in == 0) return SPIIR_OK;
+    if (!in || !out) { set_error("spiir_resample_up: NULL buffer"); return SPIIR_EINVAL; }
+    if (n_in > r->max_block) { set_error("spiir_resample_up: n_in exceeds max_block"); return SPIIR_ESTATE; }
+    if (reinterpret_cast<uintptr_t>(out) & 15u || reinterpret_cast<uintptr_t>(in) & 7u) {
+        set_error("spiir_resample_up: out must be 16-byte and in 8-byte aligned");
+        return SPIIR_EINVAL;
+    }
+    ResampArgs a;
+    a.taps = r->d_taps; a.in = in; a.out = out; a.hist = r->d_hist[r->hist_cur]; a.hist_next = r->d_hist[r->hist_cur ^ 1];
+    a.rows = r->rows; a.n_in = n_in; a.N = r->N; a.accumulate = accumulate;
+    a.tile = std::min(512, (n_in + 127) / 128 * 128);
+    const dim3 grid(r->rows, (n_in + a.tile - 1) / a.tile);
+    const size_t smem = (size_t)r->N * sizeof(float) + (size_t)(a.tile + r->N / 2) * sizeof(float2);
+    spiir_up2_kernel<<<grid, 128, smem, static_cast<cudaStream_t>(cuda_stream)>>>(a);
+    SPIIR_CUDA(cudaGetLastError());
+    r->hist_cur ^= 1;
+    return SPIIR_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,348 @@
+// spiir_filter.cuh -- sm_100a kernels for the single-rate SPIIR bank (Eq. 7 + Eq. 8).
+//
+// Mapping:
+//   * a warp task = one "group" of 32/LPT templates; LPT lanes share a template and every lane
+//     owns F filters of it, so a template's L <= F*LPT filters live in registers (a1, b0, y).
+//   * the strain window x[t0-Dpad .. t0+NT) of the CTA's stream is staged ONCE into shared
+//     memory with TMA bulk copies (cp.async.bulk + mbarrier), then replicated into four copies
+//     shifted by 0..3 samples so that every filter, whatever its delay, fetches four consecutive
+//     time steps with one aligned 16-byte LDS (row a1/a2 of SURVEY.md section 8).
+//   * Eq. 7 is evaluated with packed FP32 pairs (FFMA2/FMUL2/FADD2, sm_100a): the pair is
+//     (re, im), x and the coefficients enter as broadcast operands -- 4 packed instructions per
+//     filter-sample update instead of 8 scalar ones.
+//   * Eq. 8: per lane the F filters are summed in registers; 16 time steps are batched and summed
+//     across the LPT lanes with a transposed butterfly (xor-shuffles), which leaves every lane
+//     with a distinct slice of the 16 complex outputs -> coalesced stores, fixed summation order.
+//   * time-parallel mode (row a7): a block is cut into chunks; pass 1 runs every chunk from zero
+//     state (chunk 0 from the carried state), a carry kernel propagates s_{c+1} = a1^C s_c + e_c,
+//     pass 2 reruns every chunk from its true initial state and writes z.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace spiir {
+
+constexpr int kBatch = 16;        // time steps per reduction batch
+constexpr int kMaxWarps = 8;      // warps per CTA (launch bound 256 threads -> up to 255 registers)
+
+struct FilterArgs {
+    const float4* coef;      // [G][F][32]  (a1.re, a1.im, b0.re, b0.im), plan order
+    const int*    dly;       // [G][F][32]  delay in samples
+    float2*       state;     // [S][G][F][32] carried y (in/out)
+    float2*       chunk_st;  // chunked modes: [S][NC][G][F][32]; pass 1 writes end states, carry
+                             // turns them into initial states in place, pass 2 reads them
+    const float*  hist;      // [S][Dpad] the Dpad samples before this block, oldest first
+    float*        hist_next; // [S][Dpad] written by CTA (0, s, chunk 0)
+    const float*  x;         // [S][n]
+    float2*       z;         // [S][T][n]
+    int n, T, G, S;
+    int Dpad;                // history length, multiple of 4, >= max delay
+    int NT;                  // time-tile length (multiple of kBatch) staged per window
+    int CS;                  // stride between the shifted window copies, floats, multiple of 4
+    int NC;                  // time chunks (1 = plain streaming)
+    int C;                   // chunk length (multiple of kBatch); chunk c covers [c*C, min(n,(c+1)*C))
+    int mode;                // 0 plain, 1 chunk pass 1 (no z), 2 chunk pass 2
+    int x_aligned;           // x rows are 16-byte aligned (x pointer and n*4) -> TMA path
+    int accumulate;          // z += result instead of z = result
+};
+
+// ---------------------------------------------------------------------------------------------
+// PTX helpers: mbarrier + TMA bulk copy (global -> shared)
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint64_t* bar, int count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_LOOP:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE;\n"
+        "bra WAIT_LOOP;\n"
+        "DONE:\n"
+        "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void tma_bulk_g2s(void* dst_smem, const void* src_gmem, uint32_t bytes, uint64_t* bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(smem_u32(dst_smem)), "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+
+// ---------------------------------------------------------------------------------------------
+// Window staging.  W[i], i in [0, Dpad+len_pad): sample g = t0 - Dpad + i of stream s
+// (g < 0 -> history, 0 <= g < n -> x, else 0).  Copy s holds W shifted by s: copy_s[i] = W[i+s].
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ void stage_window(float* win, uint64_t* bar, uint32_t& parity, const FilterArgs& a,
+                                             const float* __restrict__ hist_s, const float* __restrict__ x_s,
+                                             int t0)
+{
+    const int tid = threadIdx.x, nthr = blockDim.x;
+    const int CS = a.CS, Dpad = a.Dpad, n = a.n;
+    // valid samples: i in [0, nv) where nv = Dpad + min(NT, n - t0)
+    const int nA = (t0 < Dpad) ? (Dpad - t0) : 0;           // samples taken from the history
+    const int gB = t0 - Dpad + nA;                            // first x sample (>= 0)
+    int nB = min(a.NT, n - t0) + (Dpad - nA);                 // samples taken from x
+    const int nv = nA + nB;
+    const bool use_tma = a.x_aligned != 0;
+    int nB_tma = 0;
+    if (use_tma) {
+        nB_tma = nB & ~3;
+        if (tid == 0) {
+            uint32_t bytes = (uint32_t)(nA + nB_tma) * 4u;
+            if (bytes) {
+                mbar_expect_tx(bar, bytes);
+                if (nA) tma_bulk_g2s(win, hist_s + t0, (uint32_t)nA * 4u, bar);
+                if (nB_tma) tma_bulk_g2s(win + nA, x_s + gB, (uint32_t)nB_tma * 4u, bar);
+            }
+        }
+        for (int i = nA + nB_tma + tid; i < nv; i += nthr) win[i] = x_s[gB + (i - nA)];
+    } else {
+        for (int i = tid; i < nv; i += nthr) win[i] = (i < nA) ? hist_s[t0 + i] : x_s[gB + (i - nA)];
+    }
+    for (int i = nv + tid; i < CS; i += nthr) win[i] = 0.f;   // zero tail (ragged block / shift overrun)
+    if (use_tma && (nA + nB_tma) > 0) { mbar_wait(bar, parity); parity ^= 1u; }
+    __syncthreads();
+    // shifted copies 1..3 from copy 0, 16-byte accesses only
+    const float4* w4 = reinterpret_cast<const float4*>(win);
+    const int n4 = CS >> 2;
+    for (int j = tid; j < n4 - 1; j += nthr) {
+        float4 v0 = w4[j], v1 = w4[j + 1];
+        reinterpret_cast<float4*>(win + CS)[j]     = make_float4(v0.y, v0.z, v0.w, v1.x);
+        reinterpret_cast<float4*>(win + 2 * CS)[j] = make_float4(v0.z, v0.w, v1.x, v1.y);
+        reinterpret_cast<float4*>(win + 3 * CS)[j] = make_float4(v0.w, v1.x, v1.y, v1.z);
+    }
+    if (tid == 0) {
+        const float4 zq = make_float4(0.f, 0.f, 0.f, 0.f);
+        reinterpret_cast<float4*>(win + CS)[n4 - 1] = zq;
+        reinterpret_cast<float4*>(win + 2 * CS)[n4 - 1] = zq;
+        reinterpret_cast<float4*>(win + 3 * CS)[n4 - 1] = zq;
+    }
+    __syncthreads();
+}
+
+// ---------------------------------------------------------------------------------------------
+// Transposed butterfly: Z[0..15] per lane (partial sums of 16 time steps) -> sums over the LPT
+// lanes of a template; afterwards lane j of the template holds steps [j*16/LPT, (j+1)*16/LPT)
+// (LPT = 32: lane j holds float j of the 32 floats).
+// ---------------------------------------------------------------------------------------------
+template <int N, int M>
+__device__ __forceinline__ void bfly_stage(float2* Z, int lane)
+{
+    const bool up = (lane & M) != 0;
+#pragma unroll
+    for (int i = 0; i < N / 2; ++i) {
+        float2 lo = Z[i], hi = Z[i + N / 2];
+        float2 keep = up ? hi : lo;
+        float2 send = up ? lo : hi;
+        float2 r;
+        r.x = __shfl_xor_sync(0xffffffffu, send.x, M);
+        r.y = __shfl_xor_sync(0xffffffffu, send.y, M);
+        Z[i] = __fadd2_rn(keep, r);
+    }
+}
+
+template <int LPT>
+__device__ __forceinline__ void reduce_store(float2 (&Z)[kBatch], int lane, float2* zrow, int nvalid, bool active, bool acc)
+{
+    // zrow: this lane's template row at the batch start (complex index), valid when active
+    if (LPT >= 2)  bfly_stage<16, LPT / 2>(Z, lane);
+    if (LPT >= 4)  bfly_stage<8, LPT / 4>(Z, lane);
+    if (LPT >= 8)  bfly_stage<4, LPT / 8>(Z, lane);
+    if (LPT >= 16) bfly_stage<2, LPT / 16>(Z, lane);
+    if (LPT == 32) {
+        const bool up = (lane & 1) != 0;
+        float keep = up ? Z[0].y : Z[0].x;
+        float send = up ? Z[0].x : Z[0].y;
+        float v = keep + __shfl_xor_sync(0xffffffffu, send, 1);
+        if (active && (lane >> 1) < nvalid) {
+            float* p = reinterpret_cast<float*>(zrow) + lane;
+            if (acc) v += *p;
+            *p = v;
+        }
+    } else {
+        constexpr int NV = kBatch / LPT;                  // complex values left per lane
+        const int base = (lane & (LPT - 1)) * NV;
+#pragma unroll
+        for (int i = 0; i < NV; ++i) {
+            if (active && base + i < nvalid) {
+                float2 v = Z[i];
+                if (acc) { float2 o = zrow[base + i]; v.x += o.x; v.y += o.y; }
+                zrow[base + i] = v;
+            }
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// 16 time steps of Eq. 7 for the F filters of a lane.  off4[f]: float4 index of W[Dpad + j - d_f]
+// in the right shifted copy at batch start j.
+// ---------------------------------------------------------------------------------------------
+template <int F, bool FULL, bool NOZ>
+__device__ __forceinline__ void batch_steps(const float4* __restrict__ win4, const int (&off4)[F], int j4,
+                                            const float4 (&cf)[F], float2 (&Y)[F], float2 (&Z)[kBatch], int nvalid)
+{
+#pragma unroll
+    for (int q = 0; q < kBatch / 4; ++q) {
+        float4 xv[F];
+#pragma unroll
+        for (int f = 0; f < F; ++f) xv[f] = win4[off4[f] + j4 + q];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const int step = 4 * q + u;
+            if (FULL || step < nvalid) {
+                float2 zs;
+#pragma unroll
+                for (int f = 0; f < F; ++f) {
+                    const float xs = (u == 0) ? xv[f].x : (u == 1) ? xv[f].y : (u == 2) ? xv[f].z : xv[f].w;
+                    // y' = a1*y + b0*x : (re,im) pair arithmetic
+                    float2 t = __fmul2_rn(make_float2(cf[f].z, cf[f].w), make_float2(xs, xs));
+                    t = __ffma2_rn(make_float2(cf[f].x, cf[f].x), Y[f], t);
+                    Y[f] = __ffma2_rn(make_float2(-cf[f].y, cf[f].y), make_float2(Y[f].y, Y[f].x), t);
+                    if (!NOZ) zs = (f == 0) ? Y[f] : __fadd2_rn(zs, Y[f]);
+                }
+                if (!NOZ) Z[step] = zs;
+            } else if (!NOZ) {
+                Z[step] = make_float2(0.f, 0.f);
+            }
+        }
+    }
+}
+
+template <int F, int LPT, bool NOZ>
+__global__ void __launch_bounds__(kMaxWarps * 32) spiir_filter_kernel(const FilterArgs a)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    float* win = reinterpret_cast<float*>(smem_raw);                   // 4 copies x CS floats
+    uint64_t* bar = reinterpret_cast<uint64_t*>(win + 4 * (size_t)a.CS);
+
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
+    const int s = blockIdx.y / a.NC, c = blockIdx.y % a.NC;
+    const int tc0 = c * a.C;                                            // chunk range [tc0, tc1)
+    const int tc1 = min(a.n, tc0 + a.C);
+    const float* hist_s = a.hist + (size_t)s * a.Dpad;
+    const float* x_s = a.x + (size_t)s * a.n;
+    uint32_t parity = 0;
+    if (threadIdx.x == 0) mbar_init(bar, 1);
+    __syncthreads();
+
+    // carried history for the next block (reads only hist + x: no race with other CTAs)
+    if (a.mode != 1 && blockIdx.x == 0 && c == 0) {
+        float* hn = a.hist_next + (size_t)s * a.Dpad;
+        for (int i = threadIdx.x; i < a.Dpad; i += blockDim.x) {
+            int g = a.n - a.Dpad + i;
+            hn[i] = (g >= 0) ? x_s[g] : hist_s[a.n + i];
+        }
+    }
+
+    const int ntiles = (tc1 - tc0 + a.NT - 1) / a.NT;
+    if (ntiles == 1) stage_window(win, bar, parity, a, hist_s, x_s, tc0);
+    const float4* win4 = reinterpret_cast<const float4*>(win);
+
+    constexpr int TPG = 32 / LPT;                                       // templates per group
+    for (int g0 = blockIdx.x * nwarps; g0 < a.G; g0 += gridDim.x * nwarps) {
+        const int g = g0 + warp;
+        const bool wactive = g < a.G;
+        const int t = g * TPG + lane / LPT;
+        const bool active = wactive && t < a.T;
+        float4 cf[F]; float2 Y[F]; int off4[F];
+        const size_t lbase = ((size_t)(wactive ? g : 0) * F) * 32 + lane;
+#pragma unroll
+        for (int f = 0; f < F; ++f) {
+            cf[f] = wactive ? a.coef[lbase + (size_t)f * 32] : make_float4(0.f, 0.f, 0.f, 0.f);
+            const int d = wactive ? a.dly[lbase + (size_t)f * 32] : 0;
+            const int sh = (-d) & 3;
+            off4[f] = (sh * a.CS + a.Dpad - d - sh) >> 2;
+            float2 y0 = make_float2(0.f, 0.f);
+            if (wactive) {
+                if (a.mode == 0 || (a.mode == 1 && c == 0))
+                    y0 = a.state[((size_t)s * a.G * F) * 32 + lbase + (size_t)f * 32];
+                else if (a.mode == 2)
+                    y0 = a.chunk_st[(((size_t)s * a.NC + c) * a.G * F) * 32 + lbase + (size_t)f * 32];
+            }
+            Y[f] = y0;
+        }
+        float2* zt = active ? a.z + ((size_t)s * a.T + t) * (size_t)a.n : nullptr;
+
+        for (int tile = 0; tile < ntiles; ++tile) {
+            const int t0 = tc0 + tile * a.NT;
+            const int len = min(a.NT, tc1 - t0);
+            if (ntiles > 1) { __syncthreads(); stage_window(win, bar, parity, a, hist_s, x_s, t0); }
+            const int nfull = len / kBatch;
+            float2 Z[kBatch];
+            for (int b = 0; b < nfull; ++b) {
+                batch_steps<F, true, NOZ>(win4, off4, b * (kBatch / 4), cf, Y, Z, kBatch);
+                if (!NOZ) reduce_store<LPT>(Z, lane, zt + t0 + b * kBatch, kBatch, active, a.accumulate != 0);
+            }
+            const int rem = len - nfull * kBatch;
+            if (rem > 0) {
+                batch_steps<F, false, NOZ>(win4, off4, nfull * (kBatch / 4), cf, Y, Z, rem);
+                if (!NOZ) reduce_store<LPT>(Z, lane, zt + t0 + nfull * kBatch, rem, active, a.accumulate != 0);
+            }
+        }
+        if (wactive) {
+#pragma unroll
+            for (int f = 0; f < F; ++f) {
+                if (a.mode == 0 || (a.mode == 2 && c == a.NC - 1))
+                    a.state[((size_t)s * a.G * F) * 32 + lbase + (size_t)f * 32] = Y[f];
+                else if (a.mode == 1)
+                    a.chunk_st[(((size_t)s * a.NC + c) * a.G * F) * 32 + lbase + (size_t)f * 32] = Y[f];
+            }
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Chunk carry (row a7): per filter, in place over chunk_st[s][c][i]:
+//   before: chunk_st[0] = true end state of chunk 0, chunk_st[c>=1] = zero-state end of chunk c
+//   after : chunk_st[c] = true INITIAL state of chunk c  (chunk_st[0] = carried state)
+// s_{c+1} = a1^C * s_c + e_c.  a1^C by repeated squaring in double.
+// ---------------------------------------------------------------------------------------------
+__global__ void spiir_chunk_carry_kernel(const float4* __restrict__ coef, const float2* __restrict__ state,
+                                         float2* chunk_st, int nfilt /* G*F*32 */, int S, int NC, int C)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= nfilt) return;
+    const float4 cf = coef[i];
+    double pr = 1.0, pi = 0.0, br = (double)cf.x, bi = (double)cf.y;
+    for (int e = C; e > 0; e >>= 1) {
+        if (e & 1) { double r = pr * br - pi * bi, q = pr * bi + pi * br; pr = r; pi = q; }
+        double r = br * br - bi * bi, q = 2.0 * br * bi; br = r; bi = q;
+    }
+    const float aCr = (float)pr, aCi = (float)pi;
+    for (int s = 0; s < S; ++s) {
+        float2* cs = chunk_st + (size_t)s * NC * nfilt + i;
+        float2 init = state[(size_t)s * nfilt + i];       // initial state of chunk 0
+        float2 e = cs[0];                                  // true end of chunk 0 = init of chunk 1
+        cs[0] = init;
+        float2 cur = e;
+        for (int c = 1; c < NC; ++c) {
+            float2 ec = cs[(size_t)c * nfilt];             // zero-state end of chunk c (unused for last)
+            cs[(size_t)c * nfilt] = cur;
+            float2 nxt;
+            nxt.x = fmaf(aCr, cur.x, fmaf(-aCi, cur.y, ec.x));
+            nxt.y = fmaf(aCr, cur.y, fmaf(aCi, cur.x, ec.y));
+            cur = nxt;
+        }
+    }
+}
+
+// state gather / scatter between plan order and the caller's [S][T][L] order
+__global__ void spiir_state_permute_kernel(float2* plan_state, float2* user_state, const int* __restrict__ pos,
+                                           int TL, int nfilt, int S, int to_user)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= TL) return;
+    const int p = pos[i];
+    for (int s = 0; s < S; ++s) {
+        if (to_user) user_state[(size_t)s * TL + i] = plan_state[(size_t)s * nfilt + p];
+        else plan_state[(size_t)s * nfilt + p] = user_state[(size_t)s * TL + i];
+    }
+}
+
+}  // namespace spiir

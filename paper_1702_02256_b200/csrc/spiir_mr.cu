@@ -1,0 +1,139 @@
+// spiir_mr.cu -- multirate SPIIR plan (Fig. 1).
+//   x_0 = x, x_h = down2(x_{h-1});   z_h = bank_h(x_h);
+//   acc_{H-1} = z_{H-1};  acc_{h-1} = z_{h-1} + up2(acc_h);   result acc_0 (base rate).
+// Every stage keeps its own streaming history, so consecutive calls continue one stream.
+#include <algorithm>
+#include <new>
+#include <vector>
+
+#include "spiir_internal.h"
+
+struct spiir_mr_plan {
+    int H = 0, T = 0, S = 1, max_block = 0;
+    std::vector<int> rates;
+    std::vector<spiir_plan_t*> banks;       // [H]
+    std::vector<spiir_resamp_t*> downs;     // [H-1]  x_{h} = down(x_{h-1}), rows = S
+    std::vector<spiir_resamp_t*> ups;       // [H-1]  acc_{h-1} += up(acc_h), rows = S*T
+    std::vector<float*> d_x;                // [H]    d_x[0] unused (caller's x)
+    std::vector<spiir_c64*> d_z;            // [H]    d_z[0] unused (caller's snr_out)
+};
+
+using namespace spiir;
+
+extern "C" {
+
+void spiir_mr_plan_destroy(spiir_mr_plan_t* p)
+{
+    if (!p) return;
+    for (auto b : p->banks) spiir_plan_destroy(b);
+    for (auto r : p->downs) spiir_resamp_destroy(r);
+    for (auto r : p->ups) spiir_resamp_destroy(r);
+    for (auto q : p->d_x) cudaFree(q);
+    for (auto q : p->d_z) cudaFree(q);
+    delete p;
+}
+
+spiir_status spiir_mr_plan_create(spiir_mr_plan_t** out, int n_rates, const int* rates_hz, const spiir_c64* const* a1,
+                                  const spiir_c64* const* b0, const int32_t* const* delays,
+                                  const int* n_filters_per_rate, int n_templates, const spiir_mr_opts* opts)
+{
+    if (!out) { set_error("spiir_mr_plan_create: out is NULL"); return SPIIR_EINVAL; }
+    *out = nullptr;
+    if (n_rates < 1 || n_rates > 16 || !rates_hz || !a1 || !b0 || !delays || !n_filters_per_rate || n_templates < 1) {
+        set_error("spiir_mr_plan_create: bad arguments");
+        return SPIIR_EINVAL;
+    }
+    for (int h = 1; h < n_rates; ++h)
+        if (rates_hz[h] * 2 != rates_hz[h - 1]) {
+            set_error("spiir_mr_plan_create: rates must halve (rate[%d] = %d, rate[%d] = %d)", h - 1, rates_hz[h - 1], h, rates_hz[h]);
+            return SPIIR_EINVAL;
+        }
+    spiir_mr_opts o = {1, rates_hz[0], 192, 5.0, 0.25};
+    if (opts) o = *opts;
+    if (o.n_streams < 1 || o.max_block < 1 || (o.max_block % (1 << (n_rates - 1))) != 0) {
+        set_error("spiir_mr_plan_create: max_block must be a positive multiple of 2^(n_rates-1)");
+        return SPIIR_EINVAL;
+    }
+    spiir_mr_plan* p = new (std::nothrow) spiir_mr_plan;
+    if (!p) return SPIIR_ENOMEM;
+    p->H = n_rates; p->T = n_templates; p->S = o.n_streams; p->max_block = o.max_block;
+    p->rates.assign(rates_hz, rates_hz + n_rates);
+    p->d_x.assign(n_rates, nullptr);
+    p->d_z.assign(n_rates, nullptr);
+    spiir_status rc = SPIIR_OK;
+    for (int h = 0; h < n_rates && rc == SPIIR_OK; ++h) {
+        const int nb = o.max_block >> h;
+        spiir_plan_opts po = {o.n_streams, nb, 0, 0};
+        spiir_plan_t* b = nullptr;
+        rc = spiir_plan_create(&b, a1[h], b0[h], delays[h], n_templates, n_filters_per_rate[h], rates_hz[h], &po);
+        if (rc != SPIIR_OK) break;
+        p->banks.push_back(b);
+        if (h > 0) {
+            spiir_resamp_t* d = nullptr;
+            rc = spiir_resamp_create(&d, SPIIR_DOWN2, o.n_taps, o.kaiser_beta, o.cutoff, o.n_streams, nb * 2);
+            if (rc != SPIIR_OK) break;
+            p->downs.push_back(d);
+            spiir_resamp_t* u = nullptr;
+            rc = spiir_resamp_create(&u, SPIIR_UP2, o.n_taps, o.kaiser_beta, o.cutoff, o.n_streams * n_templates, nb);
+            if (rc != SPIIR_OK) break;
+            p->ups.push_back(u);
+            cudaError_t e = cudaMalloc(&p->d_x[h], (size_t)o.n_streams * nb * sizeof(float));
+            if (e == cudaSuccess) e = cudaMalloc(&p->d_z[h], (size_t)o.n_streams * n_templates * nb * sizeof(spiir_c64));
+            if (e != cudaSuccess) { rc = cuda_fail(e, "spiir_mr_plan_create scratch"); break; }
+        }
+    }
+    if (rc != SPIIR_OK) { spiir_mr_plan_destroy(p); return rc; }
+    *out = p;
+    return SPIIR_OK;
+}
+
+spiir_status spiir_mr_filter(spiir_mr_plan_t* p, const float* x, int n, spiir_c64* snr_out, void* cuda_stream)
+{
+    if (!p || n < 0) { set_error("spiir_mr_filter: bad plan or n"); return SPIIR_EINVAL; }
+    if (n == 0) return SPIIR_OK;
+    if (!x || !snr_out) { set_error("spiir_mr_filter: NULL buffer"); return SPIIR_EINVAL; }
+    if (n % (1 << (p->H - 1)) != 0) { set_error("spiir_mr_filter: n = %d is not a multiple of 2^(H-1) = %d", n, 1 << (p->H - 1)); return SPIIR_EINVAL; }
+    if (n > p->max_block) { set_error("spiir_mr_filter: n exceeds max_block"); return SPIIR_ESTATE; }
+    if (reinterpret_cast<uintptr_t>(snr_out) & 15u) { set_error("spiir_mr_filter: snr_out must be 16-byte aligned"); return SPIIR_EINVAL; }
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    spiir_status rc;
+    const float* xh = x;
+    for (int h = 1; h < p->H; ++h) {                       // row a8: down chain
+        rc = spiir_resample_down(p->downs[h - 1], xh, n >> (h - 1), p->d_x[h], st);
+        if (rc != SPIIR_OK) return rc;
+        xh = p->d_x[h];
+    }
+    for (int h = 0; h < p->H; ++h) {                       // row a9: per-rate banks
+        rc = filter_launch(p->banks[h], h == 0 ? x : p->d_x[h], n >> h, h == 0 ? snr_out : p->d_z[h], 0, st);
+        if (rc != SPIIR_OK) return rc;
+    }
+    for (int h = p->H - 1; h >= 1; --h) {                  // row a10: up + accumulate cascade
+        rc = spiir_resample_up(p->ups[h - 1], p->d_z[h], n >> h, h == 1 ? snr_out : p->d_z[h - 1], 1, st);
+        if (rc != SPIIR_OK) return rc;
+    }
+    return SPIIR_OK;
+}
+
+spiir_status spiir_mr_plan_reset(spiir_mr_plan_t* p, void* cuda_stream)
+{
+    if (!p) { set_error("spiir_mr_plan_reset: NULL plan"); return SPIIR_EINVAL; }
+    spiir_status rc = SPIIR_OK;
+    for (auto b : p->banks) if ((rc = spiir_plan_reset(b, cuda_stream)) != SPIIR_OK) return rc;
+    for (auto r : p->downs) if ((rc = spiir_resamp_reset(r, cuda_stream)) != SPIIR_OK) return rc;
+    for (auto r : p->ups) if ((rc = spiir_resamp_reset(r, cuda_stream)) != SPIIR_OK) return rc;
+    return rc;
+}
+
+int spiir_mr_launches(const spiir_mr_plan_t* p, int n)
+{
+    if (!p || n < 1) return 0;
+    int total = 2 * (p->H - 1);
+    for (int h = 0; h < p->H; ++h) {
+        FilterGeometry g;
+        if (plan_geometry(p->banks[h], std::max(1, n >> h), &g) != SPIIR_OK) return 0;
+        total += g.launches;
+    }
+    return total;
+}
+
+}  // extern "C"
