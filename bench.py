@@ -1,0 +1,317 @@
+#!/usr/bin/env python
+"""bench.py -- SPIIR filter-sample updates/s on one B200 (BASELINE.json metric), with roofline,
+end-to-end and CPU-oracle legs.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1] [--impl ours|reference]
+
+A "step" is one streamed block of the workload through the whole hot path (spiir_filter, or
+spiir_mr_filter for config 3): for the default workload (BASELINE.json configs[1], the config the
+metric is quoted on) that is 4096 samples x 1024 templates x 256 filters = 1.07e9 Eq.-7 updates,
+with filter state and input history carried from the previous step.
+
+Timed legs:
+  value     : updates/s with the strain blocks resident in HBM; every step is bracketed by CUDA
+              events on the launching stream; an L2 flush (256 MiB write) runs between steps,
+              outside the events.
+  e2e       : the same metric through the same public call with HOST buffers: every step copies
+              its strain block from pinned host memory, filters, and copies the complex64 SNR
+              block back to pinned host memory (double-buffered on a copy stream).
+  roofline  : FP32 ALU bound: 12 flop per update / kernel time, against
+              SMs x 128 lanes x 2 flop x clocks.max.sm (DESIGN.md derives it).
+  cpu_baseline : the float64 oracle, as it stands, on this box's host cores, on a bounded sample.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "SPIIR filter-sample updates/s (templates*filters*samples/s)"
+UNIT = "updates/s"
+FLOP_PER_UPDATE = 12
+FP32_LANES_PER_SM = 128         # B200 SM: 4 sub-partitions x 32 FP32 lanes (guides/B300_MICROARCH.md)
+
+
+def _dist_env():
+    return int(os.environ.get("RANK", "0")), int(os.environ.get("LOCAL_RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
+
+
+class ClockSampler(threading.Thread):
+    """nvidia-smi clocks + throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        super().__init__(daemon=True)
+        self.index, self.rows, self._halt = index, [], threading.Event()
+
+    def run(self):
+        while not self._halt.is_set():
+            try:
+                out = subprocess.run(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                      "-i", str(self.index)], capture_output=True, text=True, timeout=5).stdout
+                self.rows.append([c.strip() for c in out.strip().split(",")])
+            except Exception:
+                pass
+            self._halt.wait(0.1)
+
+    def stop(self):
+        self._halt.set()
+        self.join(timeout=6)
+        sm, mx, reasons = [], 0.0, set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx = max(mx, float(r[1]))
+                for nm, v in zip(names, r[3:7]):
+                    if v.lower().startswith("active"):
+                        reasons.add(nm)
+            except Exception:
+                continue
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": mx or None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def make_workload(cfg: int, rank: int):
+    """BASELINE.json configs[cfg]; rank r > 0 gets its own template shard (different seed stream)."""
+    from paper_1702_02256_b200 import inputs
+    w = inputs.config(cfg)
+    if rank:
+        # independent template partition per rank (weak scaling, no data-path collective): reseed
+        from dataclasses import replace
+        banks = tuple(inputs.make_bank(tuple(w.seed_key) + (1000 + rank, h), b.a1.shape[0], b.a1.shape[1], b.rate_hz,
+                                       0.5 if cfg == 2 else 0.9, 0.999 if cfg == 2 else 0.9999, int(b.delays.max()))
+                      for h, b in enumerate(w.banks))
+        w = replace(w, banks=banks)
+    return w
+
+
+def make_plan(sp, w):
+    if len(w.banks) == 1:
+        b = w.banks[0]
+        plan = sp.Plan(b.a1, b.b0, b.delays, b.rate_hz, n_streams=w.n_streams, max_block=w.block)
+        launches = plan.launch_info(w.block)["launches"]
+    else:
+        plan = sp.MultiratePlan([(b.a1, b.b0, b.delays) for b in w.banks], [b.rate_hz for b in w.banks],
+                                n_streams=w.n_streams, max_block=w.block)
+        launches = plan.launches(w.block)
+    return plan, launches
+
+
+def oracle_sample(w, budget_updates: float):
+    """Bounded sample of the workload for the CPU legs: first T_s templates x n_b blocks."""
+    per_template_block = w.updates_per_block() / w.n_templates
+    T_s = int(min(w.n_templates, max(8, budget_updates // (2 * per_template_block))))
+    n_b = int(max(1, min(w.n_blocks, budget_updates // (T_s * per_template_block))))
+    return T_s, n_b
+
+
+def run_oracle(w, T_s: int, n_b: int):
+    """Times the oracle (float64, as it stands) on the first T_s templates for n_b blocks."""
+    import oracle
+    banks = [(b.a1[:T_s], b.b0[:T_s], b.delays[:T_s]) for b in w.banks]
+    orc = oracle.FilterOracle(*banks[0], w.n_streams) if len(banks) == 1 else oracle.MultirateOracle(banks, w.n_streams)
+    xs = [w.strain(i) for i in range(n_b)]
+    t0 = time.perf_counter()
+    for x in xs:
+        orc.filter(x)
+    dt = time.perf_counter() - t0
+    upd = w.updates_per_block() / w.n_templates * T_s * n_b
+    return upd / dt, dt, oracle.num_threads()
+
+
+def bench_reference(args):
+    rank, _, world = _dist_env()
+    if rank != 0:
+        return 0
+    w = make_workload(args.config, 0)
+    # every step is a bounded sample; the whole --steps run stays within a few minutes of CPU time
+    T_s, n_b = oracle_sample(w, min(args.cpu_budget, 8e9 / max(1, args.steps)))
+    for _ in range(min(args.warmup, 1)):
+        run_oracle(w, min(T_s, 16), 1)
+    vals, times, cores = [], [], 1
+    for _ in range(args.steps):
+        v, dt, cores = run_oracle(w, T_s, n_b)
+        vals.append(v); times.append(dt)
+    value = float(np.sum([v * t for v, t in zip(vals, times)]) / np.sum(times))
+    sample = f"first {T_s} of {w.n_templates} templates x {n_b} block(s) of {w.block} samples per step"
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": float(np.mean(times) * 1e3),
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": w.name, "sample": sample},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+def bench_ours(args):
+    import torch
+    import torch.distributed as dist
+    rank, local_rank, world = _dist_env()
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the SPIIR hot path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    import paper_1702_02256_b200 as sp
+    sp.lib()
+
+    w = make_workload(args.config, rank)
+    plan, launches = make_plan(sp, w)
+    S, T, n = w.n_streams, w.n_templates, w.block
+    upd = w.updates_per_block()
+    nblk = min(w.n_blocks, 16)
+    x_host = [torch.from_numpy(w.strain(i)).pin_memory() for i in range(nblk)]
+    x_dev = [x.cuda() for x in x_host]
+    out = torch.empty((S, T, n), dtype=torch.complex64, device="cuda")
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+    stream = torch.cuda.current_stream()
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    # ---- device-resident leg -------------------------------------------------------------------
+    for i in range(args.warmup):
+        plan.filter(x_dev[i % nblk], out)
+    barrier()
+    sampler = ClockSampler(local_rank); sampler.start()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    t_wall0 = time.perf_counter()
+    for i in range(args.steps):
+        flush.fill_(i & 0xFF)                       # L2 flush between timed steps (outside the events)
+        ev[i][0].record(stream)
+        plan.filter(x_dev[(args.warmup + i) % nblk], out)
+        ev[i][1].record(stream)
+    barrier()
+    t_wall = time.perf_counter() - t_wall0
+    clocks = sampler.stop()
+    step_ms = np.array([a.elapsed_time(b) for a, b in ev])
+    tot_ms = float(step_ms.sum())
+    if world > 1:
+        t = torch.tensor([tot_ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        tot_ms = float(t.item())
+    ms_per_step = tot_ms / args.steps
+    value = upd * world / (ms_per_step * 1e-3)
+
+    # ---- end-to-end leg: pinned host -> device -> filter -> pinned host ----------------------------
+    out2 = [torch.empty((S, T, n), dtype=torch.complex64, device="cuda") for _ in range(2)]
+    z_host = [torch.empty((S, T, n), dtype=torch.complex64).pin_memory() for _ in range(2)]
+    xin = [torch.empty((S, n), dtype=torch.float32, device="cuda") for _ in range(2)]
+    copy_stream = torch.cuda.Stream()
+    done = [torch.cuda.Event() for _ in range(2)]
+    freed = [torch.cuda.Event() for _ in range(2)]
+
+    def e2e_steps(k, first):
+        for i in range(k):
+            b = i & 1
+            stream.wait_event(freed[b])                               # out2[b] was drained to the host
+            xin[b].copy_(x_host[(first + i) % nblk], non_blocking=True)   # H2D of this step's input
+            plan.filter(xin[b], out2[b])
+            done[b].record(stream)
+            with torch.cuda.stream(copy_stream):
+                copy_stream.wait_event(done[b])
+                z_host[b].copy_(out2[b], non_blocking=True)           # D2H of this step's result
+                freed[b].record(copy_stream)
+
+    plan.reset()
+    e2e_steps(max(3, min(args.warmup, 4)), 0)
+    barrier(); copy_stream.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    e2e_steps(args.steps, 0)
+    stream.wait_stream(copy_stream)
+    e1.record(stream)
+    barrier(); copy_stream.synchronize()
+    e2e_ms = e0.elapsed_time(e1)
+    if world > 1:
+        t = torch.tensor([e2e_ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_ms = float(t.item())
+    e2e_value = upd * world * args.steps / (e2e_ms * 1e-3)
+
+    if rank == 0:
+        props = torch.cuda.get_device_properties(local_rank)
+        peaks = {}
+        try:
+            peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+        except Exception:
+            pass
+        sm_max_mhz = float(peaks.get("sm_max_mhz") or clocks.get("sm_max_mhz") or 1965.0)
+        peak_tflops = props.multi_processor_count * FP32_LANES_PER_SM * 2 * sm_max_mhz * 1e6 / 1e12
+        achieved = FLOP_PER_UPDATE * upd / (ms_per_step * 1e-3) / 1e12
+        roofline = {"bound": "alu", "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s",
+                    "frac": achieved / peak_tflops, "traffic": None,
+                    "kernel": "spiir_filter_kernel" if len(w.banks) == 1 else "spiir_filter_kernel + resamplers (whole step)",
+                    "peak_source": f"derived: {props.multi_processor_count} SMs x {FP32_LANES_PER_SM} FP32 lanes x 2 flop x "
+                                   f"{sm_max_mhz:.0f} MHz (clocks.max.sm, MEASURED_PEAKS.json); 12 flop per update (PAPER.md:88)"}
+        # FMA-pipe view: an update needs 8 FP32 lane-ops (4 packed FFMA2-class instructions); the pipe peak is
+        # SMs x 128 lane-ops per clock, so pipe utilisation = updates/s * 8 / (SMs * 128 * clock)
+        roofline["fma_pipe_frac"] = (upd / (ms_per_step * 1e-3)) * 8.0 / (props.multi_processor_count * FP32_LANES_PER_SM * sm_max_mhz * 1e6)
+        snr_bytes = S * T * n * 8
+        cpu = None
+        if not args.no_cpu:
+            T_s, n_b = oracle_sample(w, args.cpu_budget)
+            v, dt, cores = run_oracle(w, T_s, n_b)
+            cpu = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "seconds": dt,
+                   "sample": f"first {T_s} of {T} templates x {n_b} block(s) of {n} samples"}
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+                "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+                "config": {"workload": w.name, "templates_per_gpu": T, "filters_per_template": int(sum(b.a1.shape[1] for b in w.banks)),
+                           "streams": S, "block_samples": n, "rate_hz": w.banks[0].rate_hz,
+                           "updates_per_step_per_gpu": upd, "l2": "flushed between timed steps (256 MiB write)",
+                           "parallelism": f"template shards x{world}, no collective"},
+                "pct_fp32_peak": 100.0 * achieved / peak_tflops,
+                "data_seconds_per_wall_second": (n / w.banks[0].rate_hz) / (ms_per_step * 1e-3),
+                "snr_writeback_gbs": snr_bytes / (ms_per_step * 1e-3) / 1e9,
+                "step_ms_min_median_max": [float(step_ms.min()), float(np.median(step_ms)), float(step_ms.max())],
+                "wall_ms_per_step_incl_flush": t_wall * 1e3 / args.steps,
+                "clocks": clocks,
+                "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": S * n * 4, "d2h_bytes_per_step": snr_bytes,
+                        "ms_per_step": e2e_ms / args.steps},
+                "gpu_launches": launches * args.steps,
+                "roofline": roofline,
+                "cpu_baseline": cpu}
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=48)
+    ap.add_argument("--warmup", type=int, default=16)
+    ap.add_argument("--config", type=int, default=1, help="BASELINE.json configs index (default 1: the metric's config)")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--cpu-budget", type=float, default=2.2e9, help="filter-sample updates per CPU-oracle sample")
+    ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "ours":
+        args.warmup = 3
+    if args.impl == "reference":
+        return bench_reference(args)
+    return bench_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())
