@@ -196,17 +196,29 @@ __device__ __forceinline__ void batch_steps(const float4* __restrict__ win4, con
         for (int u = 0; u < 4; ++u) {
             const int step = 4 * q + u;
             if (FULL || step < nvalid) {
-                float2 zs;
+                // y' = a1*y + b0*x as (re, im) pair arithmetic; the three instructions of a filter are
+                // dependent, so they are issued breadth-first over the F filters of the lane
+                float2 t[F];
 #pragma unroll
                 for (int f = 0; f < F; ++f) {
                     const float xs = (u == 0) ? xv[f].x : (u == 1) ? xv[f].y : (u == 2) ? xv[f].z : xv[f].w;
-                    // y' = a1*y + b0*x : (re,im) pair arithmetic
-                    float2 t = __fmul2_rn(make_float2(cf[f].z, cf[f].w), make_float2(xs, xs));
-                    t = __ffma2_rn(make_float2(cf[f].x, cf[f].x), Y[f], t);
-                    Y[f] = __ffma2_rn(make_float2(-cf[f].y, cf[f].y), make_float2(Y[f].y, Y[f].x), t);
-                    if (!NOZ) zs = (f == 0) ? Y[f] : __fadd2_rn(zs, Y[f]);
+                    t[f] = __fmul2_rn(make_float2(cf[f].z, cf[f].w), make_float2(xs, xs));
                 }
-                if (!NOZ) Z[step] = zs;
+#pragma unroll
+                for (int f = 0; f < F; ++f) t[f] = __ffma2_rn(make_float2(cf[f].x, cf[f].x), Y[f], t[f]);
+                // (-yi, yr) * (ai, ai): the half-negated swap rides on the operand modifiers of FFMA2
+#pragma unroll
+                for (int f = 0; f < F; ++f) Y[f] = __ffma2_rn(make_float2(-Y[f].y, Y[f].x), make_float2(cf[f].y, cf[f].y), t[f]);
+                if (!NOZ) {
+                    // Eq. 8 within the lane: pairwise tree over the F filters (fixed order)
+#pragma unroll
+                    for (int f = 0; f < F; ++f) t[f] = Y[f];
+#pragma unroll
+                    for (int w = 1; w < F; w *= 2)
+#pragma unroll
+                        for (int f = 0; f + w < F; f += 2 * w) t[f] = __fadd2_rn(t[f], t[f + w]);
+                    Z[step] = t[0];
+                }
             } else if (!NOZ) {
                 Z[step] = make_float2(0.f, 0.f);
             }
