@@ -83,6 +83,17 @@ class ClockSampler(threading.Thread):
                 "reasons": sorted(reasons), "samples": len(sm)}
 
 
+def max_over_ranks(value: float, world: int, device="cpu") -> float:
+    """Timing rule for N > 1: every rank reports the slowest rank's device time (all_reduce MAX)."""
+    if world <= 1:
+        return float(value)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([value], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
 def make_workload(cfg: int, rank: int):
     """BASELINE.json configs[cfg]; rank r > 0 gets its own template shard (different seed stream)."""
     from paper_1702_02256_b200 import inputs
@@ -110,11 +121,19 @@ def make_plan(sp, w):
 
 
 def oracle_sample(w, budget_updates: float):
-    """Bounded sample of the workload for the CPU legs: first T_s templates x n_b blocks."""
+    """Bounded sample of the workload for the CPU legs: first T_s templates x n_b consecutive blocks
+    (the strain generator continues past the config's block count, so n_b may exceed it)."""
     per_template_block = w.updates_per_block() / w.n_templates
     T_s = int(min(w.n_templates, max(8, budget_updates // (2 * per_template_block))))
-    n_b = int(max(1, min(w.n_blocks, budget_updates // (T_s * per_template_block))))
+    n_b = int(max(1, min(256, budget_updates // (T_s * per_template_block))))
     return T_s, n_b
+
+
+def calibrated_oracle_sample(w, seconds: float):
+    """Pick a sample that keeps the oracle busy for about `seconds` on this box's cores."""
+    T0 = min(w.n_templates, 64)
+    rate, _, _ = run_oracle(w, T0, 1)
+    return oracle_sample(w, rate * seconds)
 
 
 def run_oracle(w, T_s: int, n_b: int):
@@ -137,7 +156,7 @@ def bench_reference(args):
         return 0
     w = make_workload(args.config, 0)
     # every step is a bounded sample; the whole --steps run stays within a few minutes of CPU time
-    T_s, n_b = oracle_sample(w, min(args.cpu_budget, 8e9 / max(1, args.steps)))
+    T_s, n_b = calibrated_oracle_sample(w, min(args.cpu_seconds, 150.0 / max(1, args.steps)))
     for _ in range(min(args.warmup, 1)):
         run_oracle(w, min(T_s, 16), 1)
     vals, times, cores = [], [], 1
@@ -203,10 +222,7 @@ def bench_ours(args):
     clocks = sampler.stop()
     step_ms = np.array([a.elapsed_time(b) for a, b in ev])
     tot_ms = float(step_ms.sum())
-    if world > 1:
-        t = torch.tensor([tot_ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        tot_ms = float(t.item())
+    tot_ms = max_over_ranks(tot_ms, world, "cuda")
     ms_per_step = tot_ms / args.steps
     value = upd * world / (ms_per_step * 1e-3)
 
@@ -240,10 +256,7 @@ def bench_ours(args):
     e1.record(stream)
     barrier(); copy_stream.synchronize()
     e2e_ms = e0.elapsed_time(e1)
-    if world > 1:
-        t = torch.tensor([e2e_ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_ms = float(t.item())
+    e2e_ms = max_over_ranks(e2e_ms, world, "cuda")
     e2e_value = upd * world * args.steps / (e2e_ms * 1e-3)
 
     if rank == 0:
@@ -267,7 +280,7 @@ def bench_ours(args):
         snr_bytes = S * T * n * 8
         cpu = None
         if not args.no_cpu:
-            T_s, n_b = oracle_sample(w, args.cpu_budget)
+            T_s, n_b = calibrated_oracle_sample(w, args.cpu_seconds)
             v, dt, cores = run_oracle(w, T_s, n_b)
             cpu = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "seconds": dt,
                    "sample": f"first {T_s} of {T} templates x {n_b} block(s) of {n} samples"}
@@ -303,7 +316,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=16)
     ap.add_argument("--config", type=int, default=1, help="BASELINE.json configs index (default 1: the metric's config)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--cpu-budget", type=float, default=2.2e9, help="filter-sample updates per CPU-oracle sample")
+    ap.add_argument("--cpu-seconds", type=float, default=12.0, help="target CPU time of one oracle sample")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
