@@ -108,10 +108,10 @@ def make_workload(cfg: int, rank: int):
     return w
 
 
-def make_plan(sp, w):
+def make_plan(sp, w, flags=0):
     if len(w.banks) == 1:
         b = w.banks[0]
-        plan = sp.Plan(b.a1, b.b0, b.delays, b.rate_hz, n_streams=w.n_streams, max_block=w.block)
+        plan = sp.Plan(b.a1, b.b0, b.delays, b.rate_hz, n_streams=w.n_streams, max_block=w.block, flags=flags)
         launches = plan.launch_info(w.block)["launches"]
     else:
         plan = sp.MultiratePlan([(b.a1, b.b0, b.delays) for b in w.banks], [b.rate_hz for b in w.banks],
@@ -189,7 +189,7 @@ def bench_ours(args):
     sp.lib()
 
     w = make_workload(args.config, rank)
-    plan, launches = make_plan(sp, w)
+    plan, launches = make_plan(sp, w, args.plan_flags)
     S, T, n = w.n_streams, w.n_templates, w.block
     upd = w.updates_per_block()
     nblk = min(w.n_blocks, 16)
@@ -318,6 +318,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--cpu-seconds", type=float, default=12.0, help="target CPU time of one oracle sample")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--plan-flags", type=int, default=0, help="spiir_plan_opts.flags (bit 0: skip the bank-conflict-avoiding permutation)")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3

@@ -329,6 +329,36 @@ spiir_status spiir_resample_up(spiir_resamp_t* r, const spiir_c64* in, int n_in,
         set_error("spiir_resample_up: out must be 16-byte and in 8-byte aligned");
         return SPIIR_EINVAL;
     }
+    if (r->N == 192 || r->N == 32) {
+        // register-blocked kernel, taps in the kernel parameters (constant bank)
+        UpArgs u;
+        u.in = reinterpret_cast<const float2*>(in); u.out = reinterpret_cast<float2*>(out);
+        u.hist = reinterpret_cast<const float2*>(r->d_hist[r->hist_cur]);
+        u.hist_next = reinterpret_cast<float2*>(r->d_hist[r->hist_cur ^ 1]);
+        u.rows = r->rows; u.n_in = n_in; u.accumulate = accumulate;
+        u.nseg = (n_in + kUpSegMax - 1) / kUpSegMax;
+        u.seg = ((n_in + u.nseg - 1) / u.nseg + kUpR - 1) / kUpR * kUpR;
+        u.nseg = (n_in + u.seg - 1) / u.seg;
+        u.upr = u.seg / kUpR;
+        u.rpc = std::max(1, std::min(128 / u.upr, r->rows));
+        const int half = r->N / 2;
+        const int in_stride = (u.seg + half - 1 + kUpR + 3) & ~1, out_stride = 2 * (u.seg + kUpR);
+        const size_t smem = (size_t)u.rpc * (in_stride + out_stride) * sizeof(float2);
+        const dim3 grid(u.nseg * ((r->rows + u.rpc - 1) / u.rpc));
+        cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+        if (half == 96) {
+            UpTaps<96> t;
+            for (int q = 0; q < 96; ++q) { t.t0[q] = r->taps[2 * q]; t.t1[q] = r->taps[2 * q + 1]; }
+            spiir_up2_fir_kernel<96><<<grid, 128, smem, st>>>(u, t);
+        } else {
+            UpTaps<16> t;
+            for (int q = 0; q < 16; ++q) { t.t0[q] = r->taps[2 * q]; t.t1[q] = r->taps[2 * q + 1]; }
+            spiir_up2_fir_kernel<16><<<grid, 128, smem, st>>>(u, t);
+        }
+        SPIIR_CUDA(cudaGetLastError());
+        r->hist_cur ^= 1;
+        return SPIIR_OK;
+    }
     ResampArgs a;
     a.taps = r->d_taps; a.in = in; a.out = out; a.hist = r->d_hist[r->hist_cur]; a.hist_next = r->d_hist[r->hist_cur ^ 1];
     a.rows = r->rows; a.n_in = n_in; a.N = r->N; a.accumulate = accumulate;

@@ -120,4 +120,131 @@ __global__ void __launch_bounds__(128) spiir_up2_kernel(const ResampArgs a)
     }
 }
 
+// ---------------------------------------------------------------------------------------------
+// Register-blocked up-by-2 (+ accumulate) for a compile-time tap count N = 2*HALF.
+//
+// The generic kernel above issues three shared-memory loads per two packed FMAs and is bound by the
+// LSU.  Here a thread owns R = 5 consecutive input positions m0..m0+4, i.e. 10 complex outputs in
+// 20 FP32 accumulators, and walks the R + HALF - 1 inputs they depend on once: one 8-byte LDS per
+// input feeds up to 4R FFMAs.  The taps are kernel parameters, so they live in constant bank 0 and
+// reach the FFMAs through uniform registers (LDCU), not through the vector register file or the LSU;
+// the loop is fully unrolled, which makes every tap index a compile-time constant and drops the
+// out-of-range (position, tap) pairs.
+// R = 5 is odd on purpose: lane l reads smem word pair 5l + const, and 5 is coprime with the 16
+// 8-byte banks, so the LDS.64 are conflict free.  Outputs go through shared memory to be written
+// (and, for accumulate, read) as coalesced 16-byte accesses.
+//
+// Work split: a CTA of 128 threads handles `rpc` rows x one segment of `seg` <= 640 inputs, one thread
+// per (row, 5 inputs); rpc = 128 / ceil(seg / 5) rows when the rows are short, else 1.  Small CTAs (16 KB
+// of shared memory, 48 registers) keep ~10 of them on an SM, so the load / FIR / store phases of
+// different CTAs overlap; a persistent double-buffered (cp.async) variant measured slower.
+// ---------------------------------------------------------------------------------------------
+constexpr int kUpR = 5;
+
+template <int HALF>
+struct UpTaps { float t0[HALF]; float t1[HALF]; };    // t0[q] = h[2q], t1[q] = h[2q+1]
+
+constexpr int kUpSegMax = 128 * kUpR;
+
+struct UpArgs {
+    const float2* in;        // [rows][n_in]
+    float2*       out;       // [rows][2 n_in]
+    const float2* hist;      // [rows][HALF-1]
+    float2*       hist_next;
+    int rows, n_in;
+    int seg;                 // inputs per row segment (<= kUpSegMax)
+    int nseg;                // segments per row
+    int upr;                 // units (threads) per row segment = ceil(seg / R)
+    int rpc;                 // rows per CTA
+    int accumulate;
+};
+
+template <int HALF>
+__global__ void __launch_bounds__(128, 8) spiir_up2_fir_kernel(const UpArgs a, const __grid_constant__ UpTaps<HALF> taps)
+{
+    constexpr int R = kUpR, H = HALF - 1;
+    extern __shared__ __align__(16) float2 smu[];
+    // per row slot: input segment with history [seg + H] (+ pad), then the output tile [2*seg]
+    const int in_stride = (a.seg + H + R + 3) & ~1;                     // complex words, even
+    const int out_stride = 2 * (a.seg + R);
+    float2* vin = smu;                                                  // [rpc][in_stride]
+    float2* vout = smu + (size_t)a.rpc * in_stride;                     // [rpc][out_stride]
+    const int seg_idx = blockIdx.x % a.nseg;
+    const int row0 = (blockIdx.x / a.nseg) * a.rpc;
+    const int m_base = seg_idx * a.seg;
+    const int seg_len = min(a.seg, a.n_in - m_base);
+    const int nrow = min(a.rpc, a.rows - row0);
+
+    // stage inputs: vin[slot][i] = v[row][m_base - H + i], i in [0, seg_len + H); zero beyond
+#pragma unroll 4
+    for (int sl = 0; sl < nrow; ++sl) {
+        const float2* in = a.in + (size_t)(row0 + sl) * a.n_in;
+        const float2* hist = a.hist + (size_t)(row0 + sl) * H;
+        float2* dst = vin + (size_t)sl * in_stride;
+        for (int i = threadIdx.x; i < in_stride; i += blockDim.x) {
+            const int g = m_base - H + i;
+            float2 v = make_float2(0.f, 0.f);
+            if (i < seg_len + H) {
+                if (g >= 0) v = in[g];
+                else if (H + g >= 0) v = hist[H + g];
+            }
+            dst[i] = v;
+        }
+    }
+    __syncthreads();
+
+    const int slot = threadIdx.x / a.upr, unit = threadIdx.x % a.upr;
+    if (slot < nrow && unit * R < seg_len) {
+        // inputs of this thread: local indices [unit*R, unit*R + R + H), newest = unit*R + R - 1 + H
+        const float2* vp = vin + (size_t)slot * in_stride + unit * R;
+        float2 acc0[R], acc1[R];
+#pragma unroll
+        for (int r = 0; r < R; ++r) { acc0[r] = make_float2(0.f, 0.f); acc1[r] = make_float2(0.f, 0.f); }
+#pragma unroll
+        for (int jj = 0; jj < R + H; ++jj) {
+            const float2 v = vp[R - 1 + H - jj];                        // input i = m0 + R - 1 - jj
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                const int q = r - (R - 1) + jj;                         // tap pair index of position r
+                if (q >= 0 && q < HALF) {
+                    acc0[r].x = fmaf(taps.t0[q], v.x, acc0[r].x);
+                    acc0[r].y = fmaf(taps.t0[q], v.y, acc0[r].y);
+                    acc1[r].x = fmaf(taps.t1[q], v.x, acc1[r].x);
+                    acc1[r].y = fmaf(taps.t1[q], v.y, acc1[r].y);
+                }
+            }
+        }
+        float2* op = vout + (size_t)slot * out_stride + 2 * unit * R;
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            op[2 * r] = make_float2(2.f * acc0[r].x, 2.f * acc0[r].y);
+            op[2 * r + 1] = make_float2(2.f * acc1[r].x, 2.f * acc1[r].y);
+        }
+    }
+    __syncthreads();
+
+    // coalesced write-out (16-byte accesses: even complex index, out rows are 16-byte aligned)
+#pragma unroll 4
+    for (int sl = 0; sl < nrow; ++sl) {
+        float4* o = reinterpret_cast<float4*>(a.out + (size_t)(row0 + sl) * 2 * a.n_in + 2 * m_base);
+        const float4* src = reinterpret_cast<const float4*>(vout + (size_t)sl * out_stride);
+        for (int i = threadIdx.x; i < seg_len; i += blockDim.x) {
+            float4 w = src[i];
+            if (a.accumulate) { const float4 p = o[i]; w.x += p.x; w.y += p.y; w.z += p.z; w.w += p.w; }
+            o[i] = w;
+        }
+    }
+    // carried history: last H inputs of hist ++ in (written with the first segment of a row)
+    if (seg_idx == 0 && H > 0) {
+#pragma unroll 4
+        for (int sl = 0; sl < nrow; ++sl) {
+            const int row = row0 + sl;
+            for (int i = threadIdx.x; i < H; i += blockDim.x) {
+                const int g = a.n_in - H + i;
+                a.hist_next[(size_t)row * H + i] = (g >= 0) ? a.in[(size_t)row * a.n_in + g] : a.hist[(size_t)row * H + a.n_in + i];
+            }
+        }
+    }
+}
+
 }  // namespace spiir
