@@ -305,6 +305,34 @@ spiir_status spiir_resample_down(spiir_resamp_t* r, const float* in, int n_in, f
     if (n_in == 0) return SPIIR_OK;
     if (!in || !out) { set_error("spiir_resample_down: NULL buffer"); return SPIIR_EINVAL; }
     if (n_in > r->max_block) { set_error("spiir_resample_down: n_in exceeds max_block"); return SPIIR_ESTATE; }
+    if (r->N == 192 || r->N == 32) {
+        // register-blocked kernel, taps in the kernel parameters (constant bank)
+        DownArgs d;
+        d.in = in; d.out = out;
+        d.hist = reinterpret_cast<const float*>(r->d_hist[r->hist_cur]);
+        d.hist_next = reinterpret_cast<float*>(r->d_hist[r->hist_cur ^ 1]);
+        d.rows = r->rows; d.n_in = n_in;
+        const int n_out = n_in / 2;
+        d.nseg = (n_out + kDownSegMax - 1) / kDownSegMax;
+        d.seg = ((n_out + d.nseg - 1) / d.nseg + kDownR - 1) / kDownR * kDownR;
+        d.nseg = (n_out + d.seg - 1) / d.seg;
+        const int w_len = (2 * d.seg + r->N - 1 + 2 * kDownR + 7) & ~3;
+        const size_t smem = (size_t)(w_len + d.seg) * sizeof(float);
+        const dim3 grid(d.nseg * r->rows);
+        cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+        if (r->N == 192) {
+            DownTaps<192> t;
+            memcpy(t.h, r->taps.data(), sizeof t.h);
+            spiir_down2_fir_kernel<192><<<grid, 128, smem, st>>>(d, t);
+        } else {
+            DownTaps<32> t;
+            memcpy(t.h, r->taps.data(), sizeof t.h);
+            spiir_down2_fir_kernel<32><<<grid, 128, smem, st>>>(d, t);
+        }
+        SPIIR_CUDA(cudaGetLastError());
+        r->hist_cur ^= 1;
+        return SPIIR_OK;
+    }
     ResampArgs a;
     a.taps = r->d_taps; a.in = in; a.out = out; a.hist = r->d_hist[r->hist_cur]; a.hist_next = r->d_hist[r->hist_cur ^ 1];
     a.rows = r->rows; a.n_in = n_in; a.N = r->N; a.accumulate = 0;
@@ -372,3 +400,72 @@ spiir_status spiir_resample_up(spiir_resamp_t* r, const spiir_c64* in, int n_in,
 }
 
 }  // extern "C"
+
+namespace spiir {
+
+// Row a8 in one launch: every down stage of a multirate plan (N = 192 only; the caller falls back to
+// one spiir_resample_down per stage when this returns SPIIR_EUNSUPPORTED).
+spiir_status down_chain_launch(spiir_resamp* const* downs, int nstages, const float* x, int n, float* const* xh,
+                               int n_streams, cudaStream_t st)
+{
+    if (nstages < 1 || nstages > kMaxStages || downs[0]->N != 192) return SPIIR_EUNSUPPORTED;
+    size_t words = 0;
+    for (int k = 0; k <= nstages; ++k) words += down_chain_buf_len(192, n >> k);
+    const size_t smem = words * sizeof(float);
+    if (smem > (size_t)downs[0]->dev.smem_optin) return SPIIR_EUNSUPPORTED;
+    DownChainArgs a;
+    a.x = x; a.n = n; a.nstages = nstages;
+    for (int k = 0; k < nstages; ++k) {
+        if (downs[k]->N != 192 || downs[k]->rows != n_streams) return SPIIR_EUNSUPPORTED;
+        a.xh[k] = xh[k];
+        a.hist[k] = reinterpret_cast<const float*>(downs[k]->d_hist[downs[k]->hist_cur]);
+        a.hist_next[k] = reinterpret_cast<float*>(downs[k]->d_hist[downs[k]->hist_cur ^ 1]);
+    }
+    DownTaps<192> t;
+    memcpy(t.h, downs[0]->taps.data(), sizeof t.h);
+    SPIIR_CUDA(cudaFuncSetAttribute(spiir_down_chain_kernel<192>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    spiir_down_chain_kernel<192><<<n_streams, 512, smem, st>>>(a, t);
+    SPIIR_CUDA(cudaGetLastError());
+    for (int k = 0; k < nstages; ++k) downs[k]->hist_cur ^= 1;
+    return SPIIR_OK;
+}
+
+
+// Row a10 in one launch.  ups[k] is the stage that turns the acc at n_low << k into n_low << (k+1) samples;
+// z_add[k] the per-rate SNR it is added to (the last one may be `out` itself).
+spiir_status up_chain_launch(spiir_resamp* const* ups, int nstages, const spiir_c64* z_low, int n_low,
+                             const spiir_c64* const* z_add, spiir_c64* out, int rows, cudaStream_t st)
+{
+    if (nstages < 1 || nstages > kMaxStages) return SPIIR_EUNSUPPORTED;
+    const int N = ups[0]->N;
+    if (N != 192 && N != 32) return SPIIR_EUNSUPPORTED;
+    UpChainArgs a;
+    a.z_low = reinterpret_cast<const float2*>(z_low); a.out = reinterpret_cast<float2*>(out);
+    a.rows = rows; a.n_low = n_low; a.nstages = nstages;
+    for (int k = 0; k < nstages; ++k) {
+        if (ups[k]->N != N || ups[k]->rows != rows) return SPIIR_EUNSUPPORTED;
+        a.z_add[k] = reinterpret_cast<const float2*>(z_add[k]);
+        a.hist[k] = reinterpret_cast<const float2*>(ups[k]->d_hist[ups[k]->hist_cur]);
+        a.hist_next[k] = reinterpret_cast<float2*>(ups[k]->d_hist[ups[k]->hist_cur ^ 1]);
+    }
+    a.cap_a = up_chain_buf_len(N / 2, n_low << (nstages - 1));
+    a.cap_b = up_chain_buf_len(N / 2, nstages >= 2 ? n_low << (nstages - 2) : 1);
+    const size_t smem = (size_t)(a.cap_a + a.cap_b) * sizeof(float2);
+    if (smem > (size_t)ups[0]->dev.smem_optin) return SPIIR_EUNSUPPORTED;
+    if (N == 192) {
+        UpTaps<96> t;
+        for (int q = 0; q < 96; ++q) { t.t0[q] = ups[0]->taps[2 * q]; t.t1[q] = ups[0]->taps[2 * q + 1]; }
+        SPIIR_CUDA(cudaFuncSetAttribute(spiir_up_chain_kernel<96>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        spiir_up_chain_kernel<96><<<rows, 128, smem, st>>>(a, t);
+    } else {
+        UpTaps<16> t;
+        for (int q = 0; q < 16; ++q) { t.t0[q] = ups[0]->taps[2 * q]; t.t1[q] = ups[0]->taps[2 * q + 1]; }
+        SPIIR_CUDA(cudaFuncSetAttribute(spiir_up_chain_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        spiir_up_chain_kernel<16><<<rows, 128, smem, st>>>(a, t);
+    }
+    SPIIR_CUDA(cudaGetLastError());
+    for (int k = 0; k < nstages; ++k) ups[k]->hist_cur ^= 1;
+    return SPIIR_OK;
+}
+
+}  // namespace spiir

@@ -16,6 +16,11 @@ struct spiir_mr_plan {
     std::vector<spiir_resamp_t*> ups;       // [H-1]  acc_{h-1} += up(acc_h), rows = S*T
     std::vector<float*> d_x;                // [H]    d_x[0] unused (caller's x)
     std::vector<spiir_c64*> d_z;            // [H]    d_z[0] unused (caller's snr_out)
+    // fork / join: the H banks are independent once the down chain has run, and each of them alone is
+    // too small to fill the GPU, so they are enqueued on side streams between two events
+    std::vector<cudaStream_t> side;         // [H]
+    std::vector<cudaEvent_t> ev_bank;       // [H]
+    cudaEvent_t ev_start = nullptr, ev_chain = nullptr;
 };
 
 using namespace spiir;
@@ -30,6 +35,10 @@ void spiir_mr_plan_destroy(spiir_mr_plan_t* p)
     for (auto r : p->ups) spiir_resamp_destroy(r);
     for (auto q : p->d_x) cudaFree(q);
     for (auto q : p->d_z) cudaFree(q);
+    for (auto q : p->side) if (q) cudaStreamDestroy(q);
+    for (auto q : p->ev_bank) if (q) cudaEventDestroy(q);
+    if (p->ev_start) cudaEventDestroy(p->ev_start);
+    if (p->ev_chain) cudaEventDestroy(p->ev_chain);
     delete p;
 }
 
@@ -82,6 +91,17 @@ spiir_status spiir_mr_plan_create(spiir_mr_plan_t** out, int n_rates, const int*
             if (e != cudaSuccess) { rc = cuda_fail(e, "spiir_mr_plan_create scratch"); break; }
         }
     }
+    if (rc == SPIIR_OK && n_rates > 1) {
+        p->side.assign(n_rates, nullptr);
+        p->ev_bank.assign(n_rates, nullptr);
+        cudaError_t e = cudaEventCreateWithFlags(&p->ev_start, cudaEventDisableTiming);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&p->ev_chain, cudaEventDisableTiming);
+        for (int h = 0; h < n_rates && e == cudaSuccess; ++h) {
+            e = cudaStreamCreateWithFlags(&p->side[h], cudaStreamNonBlocking);
+            if (e == cudaSuccess) e = cudaEventCreateWithFlags(&p->ev_bank[h], cudaEventDisableTiming);
+        }
+        if (e != cudaSuccess) rc = cuda_fail(e, "spiir_mr_plan_create streams");
+    }
     if (rc != SPIIR_OK) { spiir_mr_plan_destroy(p); return rc; }
     *out = p;
     return SPIIR_OK;
@@ -97,19 +117,48 @@ spiir_status spiir_mr_filter(spiir_mr_plan_t* p, const float* x, int n, spiir_c6
     if (reinterpret_cast<uintptr_t>(snr_out) & 15u) { set_error("spiir_mr_filter: snr_out must be 16-byte aligned"); return SPIIR_EINVAL; }
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     spiir_status rc;
-    const float* xh = x;
-    for (int h = 1; h < p->H; ++h) {                       // row a8: down chain
-        rc = spiir_resample_down(p->downs[h - 1], xh, n >> (h - 1), p->d_x[h], st);
+    if (p->H == 1) return filter_launch(p->banks[0], x, n, snr_out, 0, st);
+    // fork: the base-rate bank needs only x
+    SPIIR_CUDA(cudaEventRecord(p->ev_start, st));
+    SPIIR_CUDA(cudaStreamWaitEvent(p->side[0], p->ev_start, 0));
+    rc = filter_launch(p->banks[0], x, n, snr_out, 0, p->side[0]);
+    if (rc != SPIIR_OK) return rc;
+    SPIIR_CUDA(cudaEventRecord(p->ev_bank[0], p->side[0]));
+    // row a8: down chain, one launch (falls back to one launch per stage for other tap counts)
+    rc = down_chain_launch(p->downs.data(), p->H - 1, x, n, p->d_x.data() + 1, p->S, st);
+    if (rc == SPIIR_EUNSUPPORTED) {
+        const float* xh = x;
+        for (int h = 1; h < p->H; ++h) {
+            rc = spiir_resample_down(p->downs[h - 1], xh, n >> (h - 1), p->d_x[h], st);
+            if (rc != SPIIR_OK) return rc;
+            xh = p->d_x[h];
+        }
+    } else if (rc != SPIIR_OK) return rc;
+    SPIIR_CUDA(cudaEventRecord(p->ev_chain, st));
+    for (int h = 1; h < p->H; ++h) {                       // row a9: per-rate banks, side by side
+        SPIIR_CUDA(cudaStreamWaitEvent(p->side[h], p->ev_chain, 0));
+        rc = filter_launch(p->banks[h], p->d_x[h], n >> h, p->d_z[h], 0, p->side[h]);
         if (rc != SPIIR_OK) return rc;
-        xh = p->d_x[h];
+        SPIIR_CUDA(cudaEventRecord(p->ev_bank[h], p->side[h]));
     }
-    for (int h = 0; h < p->H; ++h) {                       // row a9: per-rate banks
-        rc = filter_launch(p->banks[h], h == 0 ? x : p->d_x[h], n >> h, h == 0 ? snr_out : p->d_z[h], 0, st);
-        if (rc != SPIIR_OK) return rc;
-    }
-    for (int h = p->H - 1; h >= 1; --h) {                  // row a10: up + accumulate cascade
-        rc = spiir_resample_up(p->ups[h - 1], p->d_z[h], n >> h, h == 1 ? snr_out : p->d_z[h - 1], 1, st);
-        if (rc != SPIIR_OK) return rc;
+    for (int h = 0; h < p->H; ++h) SPIIR_CUDA(cudaStreamWaitEvent(st, p->ev_bank[h], 0));   // join
+    // row a10: up + accumulate cascade, lowest rate first; one launch when the tap count has a fused kernel
+    {
+        const int nst = p->H - 1;
+        std::vector<spiir_resamp*> ups(nst);
+        std::vector<const spiir_c64*> zadd(nst);
+        for (int k = 0; k < nst; ++k) {
+            const int h = p->H - 1 - k;                   // stage k lifts rate h to rate h-1
+            ups[k] = p->ups[h - 1];
+            zadd[k] = h == 1 ? snr_out : p->d_z[h - 1];
+        }
+        rc = up_chain_launch(ups.data(), nst, p->d_z[p->H - 1], n >> (p->H - 1), zadd.data(), snr_out, p->S * p->T, st);
+        if (rc == SPIIR_EUNSUPPORTED) {
+            for (int h = p->H - 1; h >= 1; --h) {
+                rc = spiir_resample_up(p->ups[h - 1], p->d_z[h], n >> h, h == 1 ? snr_out : p->d_z[h - 1], 1, st);
+                if (rc != SPIIR_OK) return rc;
+            }
+        } else if (rc != SPIIR_OK) return rc;
     }
     return SPIIR_OK;
 }
@@ -127,7 +176,9 @@ spiir_status spiir_mr_plan_reset(spiir_mr_plan_t* p, void* cuda_stream)
 int spiir_mr_launches(const spiir_mr_plan_t* p, int n)
 {
     if (!p || n < 1) return 0;
-    int total = 2 * (p->H - 1);
+    int total = p->H > 1 ? 2 : 0;                         // fused down chain + fused up cascade
+    if (p->H > 1 && p->downs[0]->N != 192) total += p->H - 2;
+    if (p->H > 1 && p->ups[0]->N != 192 && p->ups[0]->N != 32) total += p->H - 2;
     for (int h = 0; h < p->H; ++h) {
         FilterGeometry g;
         if (plan_geometry(p->banks[h], std::max(1, n >> h), &g) != SPIIR_OK) return 0;

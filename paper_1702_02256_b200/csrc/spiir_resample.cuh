@@ -247,4 +247,248 @@ __global__ void __launch_bounds__(128, 8) spiir_up2_fir_kernel(const UpArgs a, c
     }
 }
 
+// ---------------------------------------------------------------------------------------------
+// Register-blocked down-by-2 for a compile-time tap count N (real rows).
+//
+// A thread owns R = 10 consecutive outputs; they depend on N + 2R - 2 consecutive inputs, fetched
+// with 16-byte LDS (four inputs feed up to 4R FFMAs).  Lane l starts at word 2R*l = 20 l, i.e. five
+// 16-byte chunks apart: 5 is odd, so the eight lanes of an LDS.128 phase hit eight different bank
+// groups.  Taps are kernel parameters (constant bank -> uniform registers), loop fully unrolled.
+// w[i] = u[2*m_base - (N-1) + i] is the staged input (history first); output ml of the segment is
+// sum_j h[j] * w[2*ml + N-1 - j].
+// ---------------------------------------------------------------------------------------------
+constexpr int kDownR = 10;
+constexpr int kDownSegMax = 128 * kDownR;              // outputs per row segment of the standalone kernel
+
+template <int N>
+struct DownTaps { float h[N]; };
+
+template <int N>
+__device__ __forceinline__ void down2_units(const float* __restrict__ w, int n_out, float* __restrict__ out_s,
+                                            const DownTaps<N>& taps, int first_unit, int unit_stride)
+{
+    constexpr int R = kDownR, NIN = N + 2 * R - 2, NLD = (NIN + 3) / 4;
+    for (int unit = first_unit; unit * R < n_out; unit += unit_stride) {
+        const float4* wp = reinterpret_cast<const float4*>(w + 2 * unit * R);
+        float acc[R];
+#pragma unroll
+        for (int r = 0; r < R; ++r) acc[r] = 0.f;
+#pragma unroll
+        for (int c = 0; c < NLD; ++c) {
+            const float4 v = wp[c];
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+                const int ii = 4 * c + e;                               // input index relative to the unit
+                const float x = e == 0 ? v.x : e == 1 ? v.y : e == 2 ? v.z : v.w;
+#pragma unroll
+                for (int r = 0; r < R; ++r) {
+                    const int j = 2 * r + N - 1 - ii;                   // tap of output r for this input
+                    if (ii < NIN && j >= 0 && j < N) acc[r] = fmaf(taps.h[j], x, acc[r]);
+                }
+            }
+        }
+#pragma unroll
+        for (int r = 0; r < R; ++r)
+            if (unit * R + r < n_out) out_s[unit * R + r] = acc[r];
+    }
+}
+
+struct DownArgs {
+    const float* in;         // [rows][n_in]
+    float*       out;        // [rows][n_in/2]
+    const float* hist;       // [rows][N-1]
+    float*       hist_next;
+    int rows, n_in;
+    int seg;                 // outputs per row segment (multiple of 2, <= kDownSegMax)
+    int nseg;
+};
+
+template <int N>
+__global__ void __launch_bounds__(128, 8) spiir_down2_fir_kernel(const DownArgs a, const __grid_constant__ DownTaps<N> taps)
+{
+    constexpr int H = N - 1;
+    extern __shared__ __align__(16) float smd[];
+    const int seg_idx = blockIdx.x % a.nseg, row = blockIdx.x / a.nseg;
+    const int n_out = a.n_in >> 1;
+    const int m_base = seg_idx * a.seg;
+    const int seg_len = min(a.seg, n_out - m_base);
+    const int w_len = (2 * a.seg + H + 2 * kDownR + 7) & ~3;           // staged inputs incl. over-read pad
+    float* w = smd;
+    float* out_s = smd + w_len;
+    const float* in = a.in + (size_t)row * a.n_in;
+    const float* hist = a.hist + (size_t)row * H;
+    for (int i = threadIdx.x; i < w_len; i += blockDim.x) {
+        const int g = 2 * m_base - H + i;
+        float v = 0.f;
+        if (i < 2 * seg_len + H) {
+            if (g >= 0) v = in[g];
+            else if (H + g >= 0) v = hist[H + g];
+        }
+        w[i] = v;
+    }
+    __syncthreads();
+    down2_units<N>(w, seg_len, out_s, taps, threadIdx.x, blockDim.x);
+    __syncthreads();
+    float* o = a.out + (size_t)row * n_out + m_base;
+    for (int i = threadIdx.x; i < seg_len; i += blockDim.x) o[i] = out_s[i];
+    if (seg_idx == 0) {
+        float* hn = a.hist_next + (size_t)row * H;
+        for (int i = threadIdx.x; i < H; i += blockDim.x) {
+            const int g = a.n_in - H + i;
+            hn[i] = (g >= 0) ? in[g] : hist[a.n_in + i];
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Whole down chain of the multirate plan in one launch (row a8): one CTA per stream runs the
+// stages one after the other out of shared memory.  Buffer of stage h: [history (N-1) | data n_h],
+// which is exactly the w[] layout of down2_units with m_base = 0; the outputs of a stage are the
+// data part of the next buffer and also go to global memory (the banks read them there).
+// ---------------------------------------------------------------------------------------------
+constexpr int kMaxStages = 15;
+struct DownChainArgs {
+    const float* x;                  // [S][n] base-rate input
+    float*       xh[kMaxStages];     // xh[k]: [S][n >> (k+1)] output of stage k
+    const float* hist[kMaxStages];   // [S][N-1] per stage
+    float*       hist_next[kMaxStages];
+    int n, nstages;
+};
+
+constexpr int kChainPad = 32;        // zeroed words after a buffer (the 16-byte loads of the last unit over-read)
+__host__ __device__ inline int down_chain_buf_len(int N, int n_in) { return (N - 1 + n_in + kChainPad + 3) & ~3; }
+
+template <int N>
+__global__ void __launch_bounds__(512) spiir_down_chain_kernel(const DownChainArgs a, const __grid_constant__ DownTaps<N> taps)
+{
+    constexpr int H = N - 1;
+    extern __shared__ __align__(16) float smd[];
+    const int s = blockIdx.x;
+    float* w = smd;                                                     // [history H | data n_in | pad]
+    {   // stage-0 input: history of stage 0 and the caller's block
+        const float* x = a.x + (size_t)s * a.n;
+        const float* h0 = a.hist[0] + (size_t)s * H;
+        const int len = down_chain_buf_len(N, a.n);
+        for (int i = threadIdx.x; i < len; i += blockDim.x)
+            w[i] = i < H ? h0[i] : (i < H + a.n ? x[i - H] : 0.f);
+    }
+    int n_in = a.n;
+    for (int k = 0; k < a.nstages; ++k) {
+        const int n_out = n_in >> 1;
+        float* wn = w + down_chain_buf_len(N, n_in);                    // buffer of the next stage
+        const int len_n = down_chain_buf_len(N, n_out);
+        if (k + 1 < a.nstages) {                                        // its history and zero pad
+            const float* hk = a.hist[k + 1] + (size_t)s * H;
+            for (int i = threadIdx.x; i < len_n; i += blockDim.x)
+                if (i < H || i >= H + n_out) wn[i] = i < H ? hk[i] : 0.f;
+        }
+        __syncthreads();
+        down2_units<N>(w, n_out, wn + H, taps, threadIdx.x, blockDim.x);
+        __syncthreads();
+        float* o = a.xh[k] + (size_t)s * n_out;
+        for (int i = threadIdx.x; i < n_out; i += blockDim.x) o[i] = wn[H + i];
+        // carried history of stage k: the last H words of [history | data]
+        float* hn = a.hist_next[k] + (size_t)s * H;
+        for (int i = threadIdx.x; i < H; i += blockDim.x) hn[i] = w[n_in + i];
+        w = wn; n_in = n_out;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Whole up-and-accumulate cascade of the multirate plan in one launch (row a10).  One CTA per
+// (stream, template) row climbs from the lowest rate to the base rate:
+//     acc = z_low;   for every stage: acc <- z_add[stage] + up2(acc);   out = last acc.
+// The running acc never leaves shared memory (two buffers that swap roles; buffer of a stage =
+// [history (HALF-1) | data n_in | zero pad]), only the per-rate SNR series are read from global and
+// only the base-rate result is written.  The FIR of a stage is the register-blocked loop of
+// spiir_up2_fir_kernel; the ten z_add values a thread adds to are fetched before its FIR loop, so
+// their latency hides behind ~2000 FFMAs.  z_add of the last stage may alias `out` (in place).
+// ---------------------------------------------------------------------------------------------
+struct UpChainArgs {
+    const float2* z_low;                 // [rows][n_low] output of the lowest-rate bank
+    const float2* z_add[kMaxStages];     // stage k: [rows][2 * (n_low << k)]
+    float2*       out;                   // [rows][n_low << nstages]
+    const float2* hist[kMaxStages];      // stage k: [rows][HALF-1]
+    float2*       hist_next[kMaxStages];
+    int rows, n_low, nstages;
+    int cap_a, cap_b;                    // complex words of the two buffers
+};
+
+__host__ __device__ inline int up_chain_buf_len(int half, int n_in) { return (half - 1 + n_in + kUpR + 4) & ~1; }
+
+template <int HALF>
+__global__ void __launch_bounds__(128, 7) spiir_up_chain_kernel(const UpChainArgs a, const __grid_constant__ UpTaps<HALF> taps)
+{
+    constexpr int R = kUpR, H = HALF - 1;
+    extern __shared__ __align__(16) float2 smu[];
+    const int row = blockIdx.x;
+    // stage k reads buffer (k & 1) and writes buffer ((k + 1) & 1); sizes are laid out so that the
+    // buffer holding the largest input (the last stage's) is the one of parity (nstages - 1) & 1
+    float2* buf[2];
+    buf[(a.nstages - 1) & 1] = smu;
+    buf[a.nstages & 1] = smu + a.cap_a;
+    {
+        float2* cur = buf[0];
+        const float2* zl = a.z_low + (size_t)row * a.n_low;
+        const float2* h0 = a.hist[0] + (size_t)row * H;
+        const int len = up_chain_buf_len(HALF, a.n_low);
+        for (int i = threadIdx.x; i < len; i += blockDim.x)
+            cur[i] = i < H ? h0[i] : (i < H + a.n_low ? zl[i - H] : make_float2(0.f, 0.f));
+    }
+    for (int k = 0; k < a.nstages; ++k) {
+        const int n_in = a.n_low << k;
+        const bool last = k == a.nstages - 1;
+        float2* cur = buf[k & 1];
+        float2* nxt = buf[(k + 1) & 1];
+        if (!last) {                                                    // history and zero pad of the next buffer
+            const float2* hk = a.hist[k + 1] + (size_t)row * H;
+            const int len = up_chain_buf_len(HALF, 2 * n_in);
+            for (int i = threadIdx.x; i < len; i += blockDim.x)
+                if (i < H || i >= H + 2 * n_in) nxt[i] = i < H ? hk[i] : make_float2(0.f, 0.f);
+        }
+        __syncthreads();
+        {   // carried history of this stage: the last H words of [history | data]
+            float2* hn = a.hist_next[k] + (size_t)row * H;
+            for (int i = threadIdx.x; i < H; i += blockDim.x) hn[i] = cur[n_in + i];
+        }
+        const float2* zadd = a.z_add[k] + (size_t)row * 2 * n_in;
+        float2* gout = a.out + (size_t)row * 2 * n_in;                  // used by the last stage only
+        for (int unit = threadIdx.x; unit * R < n_in; unit += blockDim.x) {
+            const int m0 = unit * R;
+            float4 old[R];
+#pragma unroll
+            for (int r = 0; r < R; ++r)
+                old[r] = m0 + r < n_in ? reinterpret_cast<const float4*>(zadd)[m0 + r] : make_float4(0.f, 0.f, 0.f, 0.f);
+            const float2* vp = cur + m0;                                // inputs [m0, m0 + R + H), newest last
+            float2 acc0[R], acc1[R];
+#pragma unroll
+            for (int r = 0; r < R; ++r) { acc0[r] = make_float2(0.f, 0.f); acc1[r] = make_float2(0.f, 0.f); }
+#pragma unroll
+            for (int jj = 0; jj < R + H; ++jj) {
+                const float2 v = vp[R - 1 + H - jj];
+#pragma unroll
+                for (int r = 0; r < R; ++r) {
+                    const int q = r - (R - 1) + jj;
+                    if (q >= 0 && q < HALF) {
+                        acc0[r].x = fmaf(taps.t0[q], v.x, acc0[r].x);
+                        acc0[r].y = fmaf(taps.t0[q], v.y, acc0[r].y);
+                        acc1[r].x = fmaf(taps.t1[q], v.x, acc1[r].x);
+                        acc1[r].y = fmaf(taps.t1[q], v.y, acc1[r].y);
+                    }
+                }
+            }
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                if (m0 + r < n_in) {
+                    const float4 w = make_float4(fmaf(2.f, acc0[r].x, old[r].x), fmaf(2.f, acc0[r].y, old[r].y),
+                                                 fmaf(2.f, acc1[r].x, old[r].z), fmaf(2.f, acc1[r].y, old[r].w));
+                    if (last) reinterpret_cast<float4*>(gout)[m0 + r] = w;
+                    else { nxt[H + 2 * (m0 + r)] = make_float2(w.x, w.y); nxt[H + 2 * (m0 + r) + 1] = make_float2(w.z, w.w); }
+                }
+            }
+        }
+        __syncthreads();
+    }
+}
+
 }  // namespace spiir
