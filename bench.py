@@ -205,9 +205,37 @@ def bench_ours(args):
             dist.barrier()
             torch.cuda.synchronize()
 
+    # One CUDA graph per resident strain block (the library keeps every ping-pong phase on the device, so
+    # a captured call can be replayed for each block of the stream); eager launches if capture fails.
+    def capture(xbuf, obuf):
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g):
+            plan.filter(xbuf, obuf)
+        return g
+
+    plan.filter(x_dev[0], out)                      # first call outside any capture (kernel attributes)
+    torch.cuda.synchronize()
+    graphs = None
+    if args.graph != "off":
+        try:
+            graphs = [capture(x_dev[i], out) for i in range(nblk)]
+        except Exception as exc:                     # pragma: no cover - depends on the driver
+            if args.graph == "on":
+                raise
+            print(f"bench.py: CUDA graph capture failed ({exc}); eager launches", file=sys.stderr)
+            graphs = None
+        plan.reset()
+        torch.cuda.synchronize()
+
+    def step(i):
+        if graphs is not None:
+            graphs[i % nblk].replay()
+        else:
+            plan.filter(x_dev[i % nblk], out)
+
     # ---- device-resident leg -------------------------------------------------------------------
     for i in range(args.warmup):
-        plan.filter(x_dev[i % nblk], out)
+        step(i)
     barrier()
     sampler = ClockSampler(local_rank); sampler.start()
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
@@ -215,7 +243,7 @@ def bench_ours(args):
     for i in range(args.steps):
         flush.fill_(i & 0xFF)                       # L2 flush between timed steps (outside the events)
         ev[i][0].record(stream)
-        plan.filter(x_dev[(args.warmup + i) % nblk], out)
+        step(args.warmup + i)
         ev[i][1].record(stream)
     barrier()
     t_wall = time.perf_counter() - t_wall0
@@ -234,12 +262,22 @@ def bench_ours(args):
     done = [torch.cuda.Event() for _ in range(2)]
     freed = [torch.cuda.Event() for _ in range(2)]
 
+    e2e_graphs = None
+    if graphs is not None:
+        try:
+            e2e_graphs = [capture(xin[b], out2[b]) for b in range(2)]
+        except Exception:                            # pragma: no cover
+            e2e_graphs = None
+
     def e2e_steps(k, first):
         for i in range(k):
             b = i & 1
             stream.wait_event(freed[b])                               # out2[b] was drained to the host
             xin[b].copy_(x_host[(first + i) % nblk], non_blocking=True)   # H2D of this step's input
-            plan.filter(xin[b], out2[b])
+            if e2e_graphs is not None:
+                e2e_graphs[b].replay()
+            else:
+                plan.filter(xin[b], out2[b])
             done[b].record(stream)
             with torch.cuda.stream(copy_stream):
                 copy_stream.wait_event(done[b])
@@ -290,6 +328,7 @@ def bench_ours(args):
                 "config": {"workload": w.name, "templates_per_gpu": T, "filters_per_template": int(sum(b.a1.shape[1] for b in w.banks)),
                            "streams": S, "block_samples": n, "rate_hz": w.banks[0].rate_hz,
                            "updates_per_step_per_gpu": upd, "l2": "flushed between timed steps (256 MiB write)",
+                           "launch": "one CUDA graph replay per step" if graphs is not None else "eager launches",
                            "parallelism": f"template shards x{world}, no collective"},
                 "pct_fp32_peak": 100.0 * achieved / peak_tflops,
                 "data_seconds_per_wall_second": (n / w.banks[0].rate_hz) / (ms_per_step * 1e-3),
@@ -318,6 +357,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--cpu-seconds", type=float, default=12.0, help="target CPU time of one oracle sample")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--graph", default="auto", choices=["auto", "on", "off"],
+                    help="replay one captured CUDA graph per step (auto: fall back to eager launches if capture fails)")
     ap.add_argument("--plan-flags", type=int, default=0, help="spiir_plan_opts.flags (bit 0: skip the bank-conflict-avoiding permutation)")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":

@@ -29,6 +29,25 @@ spiir_status device_info(DeviceInfo* out)
     return SPIIR_OK;
 }
 
+// cudaFuncSetAttribute costs several microseconds of host time: raise a kernel's dynamic shared memory
+// limit only when a launch needs more than any earlier one did (per device the limit only grows).
+static cudaError_t ensure_smem(const void* func, int bytes)
+{
+    static const void* funcs[128];
+    static int limits[128];
+    static int nfuncs = 0;
+    for (int i = 0; i < nfuncs; ++i)
+        if (funcs[i] == func) {
+            if (limits[i] >= bytes) return cudaSuccess;
+            cudaError_t e = cudaFuncSetAttribute(func, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+            if (e == cudaSuccess) limits[i] = bytes;
+            return e;
+        }
+    cudaError_t e = cudaFuncSetAttribute(func, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    if (e == cudaSuccess && nfuncs < 128) { funcs[nfuncs] = func; limits[nfuncs] = bytes; ++nfuncs; }
+    return e;
+}
+
 // ---------------------------------------------------------------------------------------------
 // kernel dispatch table: (F, LPT, NOZ) -> instantiation
 // ---------------------------------------------------------------------------------------------
@@ -90,7 +109,7 @@ spiir_status filter_launch(spiir_plan* p, const float* x, int n, spiir_c64* z, i
     if (rc != SPIIR_OK) return rc;
     FilterArgs a;
     a.coef = p->d_coef; a.dly = p->d_dly; a.state = p->d_state; a.chunk_st = p->d_chunk;
-    a.hist = p->d_hist[p->hist_cur]; a.hist_next = p->d_hist[p->hist_cur ^ 1];
+    a.hbuf[0] = p->d_hist[0]; a.hbuf[1] = p->d_hist[1]; a.phase = p->d_phase;
     a.x = x; a.z = reinterpret_cast<float2*>(z);
     a.n = n; a.T = p->T; a.G = p->G; a.S = p->S; a.Dpad = p->Dpad;
     a.NT = g.NT; a.CS = g.CS; a.NC = g.NC; a.C = g.C;
@@ -101,7 +120,7 @@ spiir_status filter_launch(spiir_plan* p, const float* x, int n, spiir_c64* z, i
         a.mode = g.NC > 1 ? pass + 1 : 0;
         filter_kernel_t k = pick_kernel(g.F, g.LPT, a.mode == 1);
         if (!k) { set_error("no kernel for F=%d LPT=%d", g.F, g.LPT); return SPIIR_EUNSUPPORTED; }
-        SPIIR_CUDA(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, g.smem_bytes));
+        SPIIR_CUDA(ensure_smem((const void*)k, g.smem_bytes));
         k<<<grid, block, g.smem_bytes, st>>>(a);
         SPIIR_CUDA(cudaGetLastError());
         if (a.mode == 1) {
@@ -110,7 +129,6 @@ spiir_status filter_launch(spiir_plan* p, const float* x, int n, spiir_c64* z, i
             SPIIR_CUDA(cudaGetLastError());
         }
     }
-    p->hist_cur ^= 1;
     return SPIIR_OK;
 }
 
@@ -124,7 +142,7 @@ void spiir_plan_destroy(spiir_plan_t* p)
 {
     if (!p) return;
     cudaFree(p->d_coef); cudaFree(p->d_dly); cudaFree(p->d_state); cudaFree(p->d_chunk);
-    cudaFree(p->d_hist[0]); cudaFree(p->d_hist[1]); cudaFree(p->d_pos);
+    cudaFree(p->d_hist[0]); cudaFree(p->d_hist[1]); cudaFree(p->d_pos); cudaFree(p->d_phase);
     delete p;
 }
 
@@ -188,6 +206,8 @@ spiir_status spiir_plan_create(spiir_plan_t** out, const spiir_c64* a1, const sp
     SPIIR_TRY(cudaMalloc(&p->d_pos, TL * sizeof(int32_t)));
     SPIIR_TRY(cudaMalloc(&p->d_hist[0], (size_t)p->S * p->Dpad * sizeof(float)));
     SPIIR_TRY(cudaMalloc(&p->d_hist[1], (size_t)p->S * p->Dpad * sizeof(float)));
+    SPIIR_TRY(cudaMalloc(&p->d_phase, 2 * sizeof(int)));
+    SPIIR_TRY(cudaMemset(p->d_phase, 0, 2 * sizeof(int)));
     if (p->NC_cap > 1) SPIIR_TRY(cudaMalloc(&p->d_chunk, (size_t)p->NC_cap * p->S * p->nfilt * sizeof(float2)));
     SPIIR_TRY(cudaMemcpy(p->d_coef, coef.data(), p->nfilt * sizeof(float4), cudaMemcpyHostToDevice));
     SPIIR_TRY(cudaMemcpy(p->d_dly, dly.data(), p->nfilt * sizeof(int32_t), cudaMemcpyHostToDevice));
@@ -221,6 +241,7 @@ spiir_status spiir_plan_reset(spiir_plan_t* p, void* cuda_stream)
     SPIIR_CUDA(cudaMemsetAsync(p->d_state, 0, (size_t)p->S * p->nfilt * sizeof(float2), st));
     SPIIR_CUDA(cudaMemsetAsync(p->d_hist[0], 0, (size_t)p->S * p->Dpad * sizeof(float), st));
     SPIIR_CUDA(cudaMemsetAsync(p->d_hist[1], 0, (size_t)p->S * p->Dpad * sizeof(float), st));
+    SPIIR_CUDA(cudaMemsetAsync(p->d_phase, 0, 2 * sizeof(int), st));
     return SPIIR_OK;
 }
 
@@ -256,7 +277,7 @@ spiir_status spiir_plan_set_state(spiir_plan_t* p, const spiir_c64* y_in, void* 
 void spiir_resamp_destroy(spiir_resamp_t* r)
 {
     if (!r) return;
-    cudaFree(r->d_taps); cudaFree(r->d_hist[0]); cudaFree(r->d_hist[1]);
+    cudaFree(r->d_taps); cudaFree(r->d_hist[0]); cudaFree(r->d_hist[1]); cudaFree(r->d_phase);
     delete r;
 }
 
@@ -282,6 +303,8 @@ spiir_status spiir_resamp_create(spiir_resamp_t** out, int direction, int n_taps
     cudaError_t e = cudaMalloc(&r->d_taps, n_taps * sizeof(float));
     if (e == cudaSuccess) e = cudaMalloc(&r->d_hist[0], hbytes);
     if (e == cudaSuccess) e = cudaMalloc(&r->d_hist[1], hbytes);
+    if (e == cudaSuccess) e = cudaMalloc(&r->d_phase, 2 * sizeof(int));
+    if (e == cudaSuccess) e = cudaMemset(r->d_phase, 0, 2 * sizeof(int));
     if (e == cudaSuccess) e = cudaMemcpy(r->d_taps, r->taps.data(), n_taps * sizeof(float), cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaMemset(r->d_hist[0], 0, hbytes);
     if (e == cudaSuccess) e = cudaMemset(r->d_hist[1], 0, hbytes);
@@ -296,6 +319,7 @@ spiir_status spiir_resamp_reset(spiir_resamp_t* r, void* cuda_stream)
     const size_t hbytes = (size_t)r->rows * std::max(1, r->H) * (r->direction == SPIIR_DOWN2 ? sizeof(float) : sizeof(float2));
     SPIIR_CUDA(cudaMemsetAsync(r->d_hist[0], 0, hbytes, static_cast<cudaStream_t>(cuda_stream)));
     SPIIR_CUDA(cudaMemsetAsync(r->d_hist[1], 0, hbytes, static_cast<cudaStream_t>(cuda_stream)));
+    SPIIR_CUDA(cudaMemsetAsync(r->d_phase, 0, 2 * sizeof(int), static_cast<cudaStream_t>(cuda_stream)));
     return SPIIR_OK;
 }
 
@@ -309,8 +333,8 @@ spiir_status spiir_resample_down(spiir_resamp_t* r, const float* in, int n_in, f
         // register-blocked kernel, taps in the kernel parameters (constant bank)
         DownArgs d;
         d.in = in; d.out = out;
-        d.hist = reinterpret_cast<const float*>(r->d_hist[r->hist_cur]);
-        d.hist_next = reinterpret_cast<float*>(r->d_hist[r->hist_cur ^ 1]);
+        d.hbuf[0] = reinterpret_cast<float*>(r->d_hist[0]); d.hbuf[1] = reinterpret_cast<float*>(r->d_hist[1]);
+        d.phase = r->d_phase;
         d.rows = r->rows; d.n_in = n_in;
         const int n_out = n_in / 2;
         d.nseg = (n_out + kDownSegMax - 1) / kDownSegMax;
@@ -330,11 +354,10 @@ spiir_status spiir_resample_down(spiir_resamp_t* r, const float* in, int n_in, f
             spiir_down2_fir_kernel<32><<<grid, 128, smem, st>>>(d, t);
         }
         SPIIR_CUDA(cudaGetLastError());
-        r->hist_cur ^= 1;
         return SPIIR_OK;
     }
     ResampArgs a;
-    a.taps = r->d_taps; a.in = in; a.out = out; a.hist = r->d_hist[r->hist_cur]; a.hist_next = r->d_hist[r->hist_cur ^ 1];
+    a.taps = r->d_taps; a.in = in; a.out = out; a.hbuf[0] = r->d_hist[0]; a.hbuf[1] = r->d_hist[1]; a.phase = r->d_phase;
     a.rows = r->rows; a.n_in = n_in; a.N = r->N; a.accumulate = 0;
     const int n_out = n_in / 2;
     a.tile = std::min(512, (n_out + 127) / 128 * 128);
@@ -342,7 +365,6 @@ spiir_status spiir_resample_down(spiir_resamp_t* r, const float* in, int n_in, f
     const size_t smem = (size_t)(r->N + 2 * (a.tile + r->N / 2)) * sizeof(float);
     spiir_down2_kernel<<<grid, 128, smem, static_cast<cudaStream_t>(cuda_stream)>>>(a);
     SPIIR_CUDA(cudaGetLastError());
-    r->hist_cur ^= 1;
     return SPIIR_OK;
 }
 
@@ -361,8 +383,8 @@ spiir_status spiir_resample_up(spiir_resamp_t* r, const spiir_c64* in, int n_in,
         // register-blocked kernel, taps in the kernel parameters (constant bank)
         UpArgs u;
         u.in = reinterpret_cast<const float2*>(in); u.out = reinterpret_cast<float2*>(out);
-        u.hist = reinterpret_cast<const float2*>(r->d_hist[r->hist_cur]);
-        u.hist_next = reinterpret_cast<float2*>(r->d_hist[r->hist_cur ^ 1]);
+        u.hbuf[0] = reinterpret_cast<float2*>(r->d_hist[0]); u.hbuf[1] = reinterpret_cast<float2*>(r->d_hist[1]);
+        u.phase = r->d_phase;
         u.rows = r->rows; u.n_in = n_in; u.accumulate = accumulate;
         u.nseg = (n_in + kUpSegMax - 1) / kUpSegMax;
         u.seg = ((n_in + u.nseg - 1) / u.nseg + kUpR - 1) / kUpR * kUpR;
@@ -384,18 +406,16 @@ spiir_status spiir_resample_up(spiir_resamp_t* r, const spiir_c64* in, int n_in,
             spiir_up2_fir_kernel<16><<<grid, 128, smem, st>>>(u, t);
         }
         SPIIR_CUDA(cudaGetLastError());
-        r->hist_cur ^= 1;
         return SPIIR_OK;
     }
     ResampArgs a;
-    a.taps = r->d_taps; a.in = in; a.out = out; a.hist = r->d_hist[r->hist_cur]; a.hist_next = r->d_hist[r->hist_cur ^ 1];
+    a.taps = r->d_taps; a.in = in; a.out = out; a.hbuf[0] = r->d_hist[0]; a.hbuf[1] = r->d_hist[1]; a.phase = r->d_phase;
     a.rows = r->rows; a.n_in = n_in; a.N = r->N; a.accumulate = accumulate;
     a.tile = std::min(512, (n_in + 127) / 128 * 128);
     const dim3 grid(r->rows, (n_in + a.tile - 1) / a.tile);
     const size_t smem = (size_t)r->N * sizeof(float) + (size_t)(a.tile + r->N / 2) * sizeof(float2);
     spiir_up2_kernel<<<grid, 128, smem, static_cast<cudaStream_t>(cuda_stream)>>>(a);
     SPIIR_CUDA(cudaGetLastError());
-    r->hist_cur ^= 1;
     return SPIIR_OK;
 }
 
@@ -418,15 +438,15 @@ spiir_status down_chain_launch(spiir_resamp* const* downs, int nstages, const fl
     for (int k = 0; k < nstages; ++k) {
         if (downs[k]->N != 192 || downs[k]->rows != n_streams) return SPIIR_EUNSUPPORTED;
         a.xh[k] = xh[k];
-        a.hist[k] = reinterpret_cast<const float*>(downs[k]->d_hist[downs[k]->hist_cur]);
-        a.hist_next[k] = reinterpret_cast<float*>(downs[k]->d_hist[downs[k]->hist_cur ^ 1]);
+        a.hbuf[k][0] = reinterpret_cast<float*>(downs[k]->d_hist[0]);
+        a.hbuf[k][1] = reinterpret_cast<float*>(downs[k]->d_hist[1]);
+        a.phase[k] = downs[k]->d_phase;
     }
     DownTaps<192> t;
     memcpy(t.h, downs[0]->taps.data(), sizeof t.h);
-    SPIIR_CUDA(cudaFuncSetAttribute(spiir_down_chain_kernel<192>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    SPIIR_CUDA(ensure_smem((const void*)spiir_down_chain_kernel<192>, (int)smem));
     spiir_down_chain_kernel<192><<<n_streams, 512, smem, st>>>(a, t);
     SPIIR_CUDA(cudaGetLastError());
-    for (int k = 0; k < nstages; ++k) downs[k]->hist_cur ^= 1;
     return SPIIR_OK;
 }
 
@@ -445,8 +465,9 @@ spiir_status up_chain_launch(spiir_resamp* const* ups, int nstages, const spiir_
     for (int k = 0; k < nstages; ++k) {
         if (ups[k]->N != N || ups[k]->rows != rows) return SPIIR_EUNSUPPORTED;
         a.z_add[k] = reinterpret_cast<const float2*>(z_add[k]);
-        a.hist[k] = reinterpret_cast<const float2*>(ups[k]->d_hist[ups[k]->hist_cur]);
-        a.hist_next[k] = reinterpret_cast<float2*>(ups[k]->d_hist[ups[k]->hist_cur ^ 1]);
+        a.hbuf[k][0] = reinterpret_cast<float2*>(ups[k]->d_hist[0]);
+        a.hbuf[k][1] = reinterpret_cast<float2*>(ups[k]->d_hist[1]);
+        a.phase[k] = ups[k]->d_phase;
     }
     a.cap_a = up_chain_buf_len(N / 2, n_low << (nstages - 1));
     a.cap_b = up_chain_buf_len(N / 2, nstages >= 2 ? n_low << (nstages - 2) : 1);
@@ -455,16 +476,15 @@ spiir_status up_chain_launch(spiir_resamp* const* ups, int nstages, const spiir_
     if (N == 192) {
         UpTaps<96> t;
         for (int q = 0; q < 96; ++q) { t.t0[q] = ups[0]->taps[2 * q]; t.t1[q] = ups[0]->taps[2 * q + 1]; }
-        SPIIR_CUDA(cudaFuncSetAttribute(spiir_up_chain_kernel<96>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        SPIIR_CUDA(ensure_smem((const void*)spiir_up_chain_kernel<96>, (int)smem));
         spiir_up_chain_kernel<96><<<rows, 128, smem, st>>>(a, t);
     } else {
         UpTaps<16> t;
         for (int q = 0; q < 16; ++q) { t.t0[q] = ups[0]->taps[2 * q]; t.t1[q] = ups[0]->taps[2 * q + 1]; }
-        SPIIR_CUDA(cudaFuncSetAttribute(spiir_up_chain_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        SPIIR_CUDA(ensure_smem((const void*)spiir_up_chain_kernel<16>, (int)smem));
         spiir_up_chain_kernel<16><<<rows, 128, smem, st>>>(a, t);
     }
     SPIIR_CUDA(cudaGetLastError());
-    for (int k = 0; k < nstages; ++k) ups[k]->hist_cur ^= 1;
     return SPIIR_OK;
 }
 

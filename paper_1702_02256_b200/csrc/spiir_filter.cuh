@@ -31,8 +31,10 @@ struct FilterArgs {
     float2*       state;     // [S][G][F][32] carried y (in/out)
     float2*       chunk_st;  // chunked modes: [S][NC][G][F][32]; pass 1 writes end states, carry
                              // turns them into initial states in place, pass 2 reads them
-    const float*  hist;      // [S][Dpad] the Dpad samples before this block, oldest first
-    float*        hist_next; // [S][Dpad] written by CTA (0, s, chunk 0)
+    float*        hbuf[2];   // [S][Dpad] input history, ping-pong: hbuf[phase] holds the Dpad samples before
+                             // this block (oldest first), hbuf[phase ^ 1] is written by CTA (0, s, chunk 0)
+    int*          phase;     // device words {phase, arrivals}: which buffer is current is decided on the
+                             // device, so that every call enqueues identical work (CUDA-graph replayable)
     const float*  x;         // [S][n]
     float2*       z;         // [S][T][n]
     int n, T, G, S;
@@ -45,6 +47,23 @@ struct FilterArgs {
     int x_aligned;           // x rows are 16-byte aligned (x pointer and n*4) -> TMA path
     int accumulate;          // z += result instead of z = result
 };
+
+// ---------------------------------------------------------------------------------------------
+// Ping-pong phase kept on the device.  A kernel reads w[0] when it starts; the CTA that finishes last
+// (arrival counter w[1]) flips it, so no CTA can observe the flip of its own launch.
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ int phase_read(const int* w) { return *reinterpret_cast<const volatile int*>(w) & 1; }
+__device__ __forceinline__ bool last_cta_arrives(int* w, int total_ctas)
+{
+    __syncthreads();
+    bool last = false;
+    if (threadIdx.x == 0) {
+        __threadfence();
+        last = atomicAdd(w + 1, 1) == total_ctas - 1;
+        if (last) w[1] = 0;
+    }
+    return last;                                     // meaningful in thread 0 only
+}
 
 // ---------------------------------------------------------------------------------------------
 // PTX helpers: mbarrier + TMA bulk copy (global -> shared)
@@ -237,7 +256,8 @@ __global__ void __launch_bounds__(kMaxWarps * 32) spiir_filter_kernel(const Filt
     const int s = blockIdx.y / a.NC, c = blockIdx.y % a.NC;
     const int tc0 = c * a.C;                                            // chunk range [tc0, tc1)
     const int tc1 = min(a.n, tc0 + a.C);
-    const float* hist_s = a.hist + (size_t)s * a.Dpad;
+    const int ph = phase_read(a.phase);
+    const float* hist_s = a.hbuf[ph] + (size_t)s * a.Dpad;
     const float* x_s = a.x + (size_t)s * a.n;
     uint32_t parity = 0;
     if (threadIdx.x == 0) mbar_init(bar, 1);
@@ -245,7 +265,7 @@ __global__ void __launch_bounds__(kMaxWarps * 32) spiir_filter_kernel(const Filt
 
     // carried history for the next block (reads only hist + x: no race with other CTAs)
     if (a.mode != 1 && blockIdx.x == 0 && c == 0) {
-        float* hn = a.hist_next + (size_t)s * a.Dpad;
+        float* hn = a.hbuf[ph ^ 1] + (size_t)s * a.Dpad;
         for (int i = threadIdx.x; i < a.Dpad; i += blockDim.x) {
             int g = a.n - a.Dpad + i;
             hn[i] = (g >= 0) ? x_s[g] : hist_s[a.n + i];
@@ -307,6 +327,7 @@ __global__ void __launch_bounds__(kMaxWarps * 32) spiir_filter_kernel(const Filt
             }
         }
     }
+    if (a.mode != 1 && last_cta_arrives(a.phase, gridDim.x * gridDim.y)) a.phase[0] = ph ^ 1;
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -329,17 +350,23 @@ __global__ void spiir_chunk_carry_kernel(const float4* __restrict__ coef, const 
     const float aCr = (float)pr, aCi = (float)pi;
     for (int s = 0; s < S; ++s) {
         float2* cs = chunk_st + (size_t)s * NC * nfilt + i;
-        float2 init = state[(size_t)s * nfilt + i];       // initial state of chunk 0
-        float2 e = cs[0];                                  // true end of chunk 0 = init of chunk 1
-        cs[0] = init;
-        float2 cur = e;
-        for (int c = 1; c < NC; ++c) {
-            float2 ec = cs[(size_t)c * nfilt];             // zero-state end of chunk c (unused for last)
-            cs[(size_t)c * nfilt] = cur;
-            float2 nxt;
-            nxt.x = fmaf(aCr, cur.x, fmaf(-aCi, cur.y, ec.x));
-            nxt.y = fmaf(aCr, cur.y, fmaf(aCi, cur.x, ec.y));
-            cur = nxt;
+        float2 cur = cs[0];                                // true end of chunk 0 = initial state of chunk 1
+        cs[0] = state[(size_t)s * nfilt + i];              // initial state of chunk 0
+        // the zero-state ends are fetched eight at a time so that their load latencies overlap
+        for (int c0 = 1; c0 < NC; c0 += 8) {
+            float2 ec[8];
+#pragma unroll
+            for (int j = 0; j < 8; ++j) ec[j] = c0 + j < NC ? cs[(size_t)(c0 + j) * nfilt] : make_float2(0.f, 0.f);
+#pragma unroll
+            for (int j = 0; j < 8; ++j) {
+                if (c0 + j < NC) {
+                    cs[(size_t)(c0 + j) * nfilt] = cur;
+                    float2 nxt;
+                    nxt.x = fmaf(aCr, cur.x, fmaf(-aCi, cur.y, ec[j].x));
+                    nxt.y = fmaf(aCr, cur.y, fmaf(aCi, cur.x, ec[j].y));
+                    cur = nxt;
+                }
+            }
         }
     }
 }

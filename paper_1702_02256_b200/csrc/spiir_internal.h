@@ -67,7 +67,7 @@ struct spiir_plan {
     float2* d_state = nullptr;
     float2* d_chunk = nullptr;
     float* d_hist[2] = {nullptr, nullptr};
-    int hist_cur = 0;
+    int* d_phase = nullptr;           // {phase, arrivals}: which d_hist is current (flipped on the device)
     int32_t* d_pos = nullptr;
     double conflict_degree = 0.0;
 };
@@ -77,7 +77,7 @@ struct spiir_resamp {
     int H = 0;                        // history samples per row
     float* d_taps = nullptr;
     void* d_hist[2] = {nullptr, nullptr};
-    int hist_cur = 0;
+    int* d_phase = nullptr;           // {phase, arrivals}
     std::vector<float> taps;
     spiir::DeviceInfo dev;
 };

@@ -10,6 +10,8 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include "spiir_filter.cuh"   // phase_read / last_cta_arrives
+
 namespace spiir {
 
 constexpr int kMaxTaps = 1024;
@@ -18,8 +20,8 @@ struct ResampArgs {
     const float* taps;      // [N] float32 taps (device)
     const void*  in;        // down: float [rows][n_in]; up: float2 [rows][n_in]
     void*        out;       // down: float [rows][n_in/2]; up: float2 [rows][2 n_in]
-    const void*  hist;      // down: float [rows][N-1]; up: float2 [rows][N/2-1]
-    void*        hist_next;
+    void*        hbuf[2];   // down: float [rows][N-1]; up: float2 [rows][N/2-1]; ping-pong, hbuf[phase] is current
+    int*         phase;     // device words {phase, arrivals} (see spiir_filter.cuh)
     int rows, n_in, N;
     int tile;               // down: outputs per CTA; up: inputs per CTA
     int accumulate;         // up only
@@ -39,8 +41,9 @@ __global__ void __launch_bounds__(128) spiir_down2_kernel(const ResampArgs a)
     float* taps = sm;                               // [N]
     float* ue = taps + N;                           // ue[i] = u[2(m0 - half + i)],     i in [0, tm+half)
     float* uo = ue + (a.tile + half);               // uo[i] = u[2(m0 - half + i) + 1]
+    const int ph = phase_read(a.phase);
     const float* in = reinterpret_cast<const float*>(a.in) + (size_t)row * a.n_in;
-    const float* hist = reinterpret_cast<const float*>(a.hist) + (size_t)row * H;
+    const float* hist = reinterpret_cast<const float*>(a.hbuf[ph]) + (size_t)row * H;
     for (int i = threadIdx.x; i < N; i += blockDim.x) taps[i] = a.taps[i];
     const int base = 2 * (m0 - half);               // first input sample staged (may be < 0 -> history)
     for (int i = threadIdx.x; i < 2 * (tm + half); i += blockDim.x) {
@@ -63,12 +66,13 @@ __global__ void __launch_bounds__(128) spiir_down2_kernel(const ResampArgs a)
         reinterpret_cast<float*>(a.out)[(size_t)row * n_out + m0 + ml] = acc0 + acc1;
     }
     if (blockIdx.y == 0 && H > 0) {                 // carried history: last H samples of hist ++ in
-        float* hn = reinterpret_cast<float*>(a.hist_next) + (size_t)row * H;
+        float* hn = reinterpret_cast<float*>(a.hbuf[ph ^ 1]) + (size_t)row * H;
         for (int i = threadIdx.x; i < H; i += blockDim.x) {
             const int g = a.n_in - H + i;
             hn[i] = (g >= 0) ? in[g] : hist[a.n_in + i];
         }
     }
+    if (last_cta_arrives(a.phase, gridDim.x * gridDim.y)) a.phase[0] = ph ^ 1;
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -85,8 +89,9 @@ __global__ void __launch_bounds__(128) spiir_up2_kernel(const ResampArgs a)
     float* tp0 = sm;                                // h[2q]
     float* tp1 = sm + half;                         // h[2q+1]
     float2* vs = reinterpret_cast<float2*>(sm + N); // vs[i] = v[m0 - H + i], i in [0, tm+H)
+    const int ph = phase_read(a.phase);
     const float2* in = reinterpret_cast<const float2*>(a.in) + (size_t)row * a.n_in;
-    const float2* hist = reinterpret_cast<const float2*>(a.hist) + (size_t)row * H;
+    const float2* hist = reinterpret_cast<const float2*>(a.hbuf[ph]) + (size_t)row * H;
     for (int i = threadIdx.x; i < half; i += blockDim.x) { tp0[i] = a.taps[2 * i]; tp1[i] = a.taps[2 * i + 1]; }
     for (int i = threadIdx.x; i < tm + H; i += blockDim.x) {
         const int g = m0 - H + i;
@@ -112,12 +117,13 @@ __global__ void __launch_bounds__(128) spiir_up2_kernel(const ResampArgs a)
         *o = w;
     }
     if (blockIdx.y == 0 && H > 0) {
-        float2* hn = reinterpret_cast<float2*>(a.hist_next) + (size_t)row * H;
+        float2* hn = reinterpret_cast<float2*>(a.hbuf[ph ^ 1]) + (size_t)row * H;
         for (int i = threadIdx.x; i < H; i += blockDim.x) {
             const int g = a.n_in - H + i;
             hn[i] = (g >= 0) ? in[g] : hist[a.n_in + i];
         }
     }
+    if (last_cta_arrives(a.phase, gridDim.x * gridDim.y)) a.phase[0] = ph ^ 1;
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -149,8 +155,8 @@ constexpr int kUpSegMax = 128 * kUpR;
 struct UpArgs {
     const float2* in;        // [rows][n_in]
     float2*       out;       // [rows][2 n_in]
-    const float2* hist;      // [rows][HALF-1]
-    float2*       hist_next;
+    float2*       hbuf[2];   // [rows][HALF-1] ping-pong, hbuf[phase] is current
+    int*          phase;
     int rows, n_in;
     int seg;                 // inputs per row segment (<= kUpSegMax)
     int nseg;                // segments per row
@@ -174,12 +180,15 @@ __global__ void __launch_bounds__(128, 8) spiir_up2_fir_kernel(const UpArgs a, c
     const int m_base = seg_idx * a.seg;
     const int seg_len = min(a.seg, a.n_in - m_base);
     const int nrow = min(a.rpc, a.rows - row0);
+    const int ph = phase_read(a.phase);
+    const float2* hcur = a.hbuf[ph];
+    float2* hnext = a.hbuf[ph ^ 1];
 
     // stage inputs: vin[slot][i] = v[row][m_base - H + i], i in [0, seg_len + H); zero beyond
 #pragma unroll 4
     for (int sl = 0; sl < nrow; ++sl) {
         const float2* in = a.in + (size_t)(row0 + sl) * a.n_in;
-        const float2* hist = a.hist + (size_t)(row0 + sl) * H;
+        const float2* hist = hcur + (size_t)(row0 + sl) * H;
         float2* dst = vin + (size_t)sl * in_stride;
         for (int i = threadIdx.x; i < in_stride; i += blockDim.x) {
             const int g = m_base - H + i;
@@ -241,10 +250,11 @@ __global__ void __launch_bounds__(128, 8) spiir_up2_fir_kernel(const UpArgs a, c
             const int row = row0 + sl;
             for (int i = threadIdx.x; i < H; i += blockDim.x) {
                 const int g = a.n_in - H + i;
-                a.hist_next[(size_t)row * H + i] = (g >= 0) ? a.in[(size_t)row * a.n_in + g] : a.hist[(size_t)row * H + a.n_in + i];
+                hnext[(size_t)row * H + i] = (g >= 0) ? a.in[(size_t)row * a.n_in + g] : hcur[(size_t)row * H + a.n_in + i];
             }
         }
     }
+    if (last_cta_arrives(a.phase, gridDim.x)) a.phase[0] = ph ^ 1;
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -296,8 +306,8 @@ __device__ __forceinline__ void down2_units(const float* __restrict__ w, int n_o
 struct DownArgs {
     const float* in;         // [rows][n_in]
     float*       out;        // [rows][n_in/2]
-    const float* hist;       // [rows][N-1]
-    float*       hist_next;
+    float*       hbuf[2];    // [rows][N-1] ping-pong, hbuf[phase] is current
+    int*         phase;
     int rows, n_in;
     int seg;                 // outputs per row segment (multiple of 2, <= kDownSegMax)
     int nseg;
@@ -315,8 +325,9 @@ __global__ void __launch_bounds__(128, 8) spiir_down2_fir_kernel(const DownArgs 
     const int w_len = (2 * a.seg + H + 2 * kDownR + 7) & ~3;           // staged inputs incl. over-read pad
     float* w = smd;
     float* out_s = smd + w_len;
+    const int ph = phase_read(a.phase);
     const float* in = a.in + (size_t)row * a.n_in;
-    const float* hist = a.hist + (size_t)row * H;
+    const float* hist = a.hbuf[ph] + (size_t)row * H;
     for (int i = threadIdx.x; i < w_len; i += blockDim.x) {
         const int g = 2 * m_base - H + i;
         float v = 0.f;
@@ -332,12 +343,13 @@ __global__ void __launch_bounds__(128, 8) spiir_down2_fir_kernel(const DownArgs 
     float* o = a.out + (size_t)row * n_out + m_base;
     for (int i = threadIdx.x; i < seg_len; i += blockDim.x) o[i] = out_s[i];
     if (seg_idx == 0) {
-        float* hn = a.hist_next + (size_t)row * H;
+        float* hn = a.hbuf[ph ^ 1] + (size_t)row * H;
         for (int i = threadIdx.x; i < H; i += blockDim.x) {
             const int g = a.n_in - H + i;
             hn[i] = (g >= 0) ? in[g] : hist[a.n_in + i];
         }
     }
+    if (last_cta_arrives(a.phase, gridDim.x)) a.phase[0] = ph ^ 1;
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -350,8 +362,8 @@ constexpr int kMaxStages = 15;
 struct DownChainArgs {
     const float* x;                  // [S][n] base-rate input
     float*       xh[kMaxStages];     // xh[k]: [S][n >> (k+1)] output of stage k
-    const float* hist[kMaxStages];   // [S][N-1] per stage
-    float*       hist_next[kMaxStages];
+    float*       hbuf[kMaxStages][2];   // [S][N-1] per stage, ping-pong
+    int*         phase[kMaxStages];     // per stage {phase, arrivals}; arrivals of stage 0 count this kernel's CTAs
     int n, nstages;
 };
 
@@ -367,7 +379,7 @@ __global__ void __launch_bounds__(512) spiir_down_chain_kernel(const DownChainAr
     float* w = smd;                                                     // [history H | data n_in | pad]
     {   // stage-0 input: history of stage 0 and the caller's block
         const float* x = a.x + (size_t)s * a.n;
-        const float* h0 = a.hist[0] + (size_t)s * H;
+        const float* h0 = a.hbuf[0][phase_read(a.phase[0])] + (size_t)s * H;
         const int len = down_chain_buf_len(N, a.n);
         for (int i = threadIdx.x; i < len; i += blockDim.x)
             w[i] = i < H ? h0[i] : (i < H + a.n ? x[i - H] : 0.f);
@@ -378,7 +390,7 @@ __global__ void __launch_bounds__(512) spiir_down_chain_kernel(const DownChainAr
         float* wn = w + down_chain_buf_len(N, n_in);                    // buffer of the next stage
         const int len_n = down_chain_buf_len(N, n_out);
         if (k + 1 < a.nstages) {                                        // its history and zero pad
-            const float* hk = a.hist[k + 1] + (size_t)s * H;
+            const float* hk = a.hbuf[k + 1][phase_read(a.phase[k + 1])] + (size_t)s * H;
             for (int i = threadIdx.x; i < len_n; i += blockDim.x)
                 if (i < H || i >= H + n_out) wn[i] = i < H ? hk[i] : 0.f;
         }
@@ -388,10 +400,12 @@ __global__ void __launch_bounds__(512) spiir_down_chain_kernel(const DownChainAr
         float* o = a.xh[k] + (size_t)s * n_out;
         for (int i = threadIdx.x; i < n_out; i += blockDim.x) o[i] = wn[H + i];
         // carried history of stage k: the last H words of [history | data]
-        float* hn = a.hist_next[k] + (size_t)s * H;
+        float* hn = a.hbuf[k][phase_read(a.phase[k]) ^ 1] + (size_t)s * H;
         for (int i = threadIdx.x; i < H; i += blockDim.x) hn[i] = w[n_in + i];
         w = wn; n_in = n_out;
     }
+    if (last_cta_arrives(a.phase[0], gridDim.x))
+        for (int k = 0; k < a.nstages; ++k) a.phase[k][0] ^= 1;
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -408,8 +422,8 @@ struct UpChainArgs {
     const float2* z_low;                 // [rows][n_low] output of the lowest-rate bank
     const float2* z_add[kMaxStages];     // stage k: [rows][2 * (n_low << k)]
     float2*       out;                   // [rows][n_low << nstages]
-    const float2* hist[kMaxStages];      // stage k: [rows][HALF-1]
-    float2*       hist_next[kMaxStages];
+    float2*       hbuf[kMaxStages][2];   // stage k: [rows][HALF-1], ping-pong
+    int*          phase[kMaxStages];     // per stage {phase, arrivals}; arrivals of stage 0 count this kernel's CTAs
     int rows, n_low, nstages;
     int cap_a, cap_b;                    // complex words of the two buffers
 };
@@ -430,7 +444,7 @@ __global__ void __launch_bounds__(128, 7) spiir_up_chain_kernel(const UpChainArg
     {
         float2* cur = buf[0];
         const float2* zl = a.z_low + (size_t)row * a.n_low;
-        const float2* h0 = a.hist[0] + (size_t)row * H;
+        const float2* h0 = a.hbuf[0][phase_read(a.phase[0])] + (size_t)row * H;
         const int len = up_chain_buf_len(HALF, a.n_low);
         for (int i = threadIdx.x; i < len; i += blockDim.x)
             cur[i] = i < H ? h0[i] : (i < H + a.n_low ? zl[i - H] : make_float2(0.f, 0.f));
@@ -441,14 +455,14 @@ __global__ void __launch_bounds__(128, 7) spiir_up_chain_kernel(const UpChainArg
         float2* cur = buf[k & 1];
         float2* nxt = buf[(k + 1) & 1];
         if (!last) {                                                    // history and zero pad of the next buffer
-            const float2* hk = a.hist[k + 1] + (size_t)row * H;
+            const float2* hk = a.hbuf[k + 1][phase_read(a.phase[k + 1])] + (size_t)row * H;
             const int len = up_chain_buf_len(HALF, 2 * n_in);
             for (int i = threadIdx.x; i < len; i += blockDim.x)
                 if (i < H || i >= H + 2 * n_in) nxt[i] = i < H ? hk[i] : make_float2(0.f, 0.f);
         }
         __syncthreads();
         {   // carried history of this stage: the last H words of [history | data]
-            float2* hn = a.hist_next[k] + (size_t)row * H;
+            float2* hn = a.hbuf[k][phase_read(a.phase[k]) ^ 1] + (size_t)row * H;
             for (int i = threadIdx.x; i < H; i += blockDim.x) hn[i] = cur[n_in + i];
         }
         const float2* zadd = a.z_add[k] + (size_t)row * 2 * n_in;
@@ -489,6 +503,8 @@ __global__ void __launch_bounds__(128, 7) spiir_up_chain_kernel(const UpChainArg
         }
         __syncthreads();
     }
+    if (last_cta_arrives(a.phase[0], gridDim.x))
+        for (int k = 0; k < a.nstages; ++k) a.phase[k][0] ^= 1;
 }
 
 }  // namespace spiir

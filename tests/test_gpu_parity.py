@@ -322,3 +322,49 @@ def test_kaiser_taps_match_oracle_design(sp, oracle_mod):
     h = sp.spiir_kaiser_taps(192, 5.0, 0.25)
     _, h32 = oracle_mod.kaiser_taps(192, 5.0, 0.25)
     assert np.max(np.abs(h.astype(np.float64) - h32.astype(np.float64)) / np.spacing(np.abs(h32)).astype(np.float64)) <= 1.0
+
+
+# ------------------------------------------------------------------------------------------------
+# CUDA graphs: the ping-pong phase of every carried history lives on the device, so one captured
+# call can be replayed for every block of a stream
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("kind", ["few_filter_chunked", "many_filter", "multirate"])
+def test_cuda_graph_replay_continues_the_stream(sp, oracle_mod, kind):
+    import torch
+    inp = _inputs()
+    if kind == "multirate":
+        w = inp.config(3, n_templates=12, n_blocks=5)
+        banks = [(b.a1, b.b0, b.delays) for b in w.banks]
+        plan = sp.MultiratePlan(banks, [b.rate_hz for b in w.banks], max_block=w.block)
+        orc = oracle_mod.MultirateOracle(banks)
+        T = 12
+    else:
+        w = inp.config(2, n_templates=300, n_filters=8, n_blocks=5) if kind == "few_filter_chunked" else \
+            inp.config(1, n_templates=20, n_blocks=5)
+        b = w.banks[0]
+        plan = sp.Plan(b.a1, b.b0, b.delays, b.rate_hz, max_block=w.block)
+        orc = oracle_mod.FilterOracle(b.a1, b.b0, b.delays)
+        T = b.a1.shape[0]
+    xs = [w.strain(i) for i in range(5)]
+    x_static = torch.zeros((1, w.block), dtype=torch.float32, device="cuda")
+    out_static = torch.zeros((1, T, w.block), dtype=torch.complex64, device="cuda")
+    # warm-up outside the capture (sets kernel attributes), then start the stream again
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(side):
+        plan.filter(x_static, out_static)
+    torch.cuda.current_stream().wait_stream(side)
+    plan.reset()
+    torch.cuda.synchronize()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g):
+        plan.filter(x_static, out_static)
+    plan.reset()                      # whatever the capture did to host-side bookkeeping, the device state restarts
+    outs = []
+    for x in xs:
+        x_static.copy_(torch.from_numpy(x))
+        g.replay()
+        outs.append(out_static.cpu().numpy().copy())
+    z = np.concatenate(outs, -1)
+    ref = stream_oracle(orc, xs)
+    assert_parity(z, ref, f"graph replay {kind}")
