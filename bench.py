@@ -94,10 +94,10 @@ def max_over_ranks(value: float, world: int, device="cpu") -> float:
     return float(t.item())
 
 
-def make_workload(cfg: int, rank: int):
+def make_workload(cfg: int, rank: int, n_filters: int = 0):
     """BASELINE.json configs[cfg]; rank r > 0 gets its own template shard (different seed stream)."""
     from paper_1702_02256_b200 import inputs
-    w = inputs.config(cfg)
+    w = inputs.config(cfg, n_filters=n_filters or None) if cfg == 2 else inputs.config(cfg)
     if rank:
         # independent template partition per rank (weak scaling, no data-path collective): reseed
         from dataclasses import replace
@@ -108,10 +108,11 @@ def make_workload(cfg: int, rank: int):
     return w
 
 
-def make_plan(sp, w, flags=0):
+def make_plan(sp, w, flags=0, time_chunks=0):
     if len(w.banks) == 1:
         b = w.banks[0]
-        plan = sp.Plan(b.a1, b.b0, b.delays, b.rate_hz, n_streams=w.n_streams, max_block=w.block, flags=flags)
+        plan = sp.Plan(b.a1, b.b0, b.delays, b.rate_hz, n_streams=w.n_streams, max_block=w.block, flags=flags,
+                       time_chunks=time_chunks)
         launches = plan.launch_info(w.block)["launches"]
     else:
         plan = sp.MultiratePlan([(b.a1, b.b0, b.delays) for b in w.banks], [b.rate_hz for b in w.banks],
@@ -154,7 +155,7 @@ def bench_reference(args):
     rank, _, world = _dist_env()
     if rank != 0:
         return 0
-    w = make_workload(args.config, 0)
+    w = make_workload(args.config, 0, args.filters)
     # every step is a bounded sample; the whole --steps run stays within a few minutes of CPU time
     T_s, n_b = calibrated_oracle_sample(w, min(args.cpu_seconds, 150.0 / max(1, args.steps)))
     for _ in range(min(args.warmup, 1)):
@@ -188,8 +189,8 @@ def bench_ours(args):
     import paper_1702_02256_b200 as sp
     sp.lib()
 
-    w = make_workload(args.config, rank)
-    plan, launches = make_plan(sp, w, args.plan_flags)
+    w = make_workload(args.config, rank, args.filters)
+    plan, launches = make_plan(sp, w, args.plan_flags, args.time_chunks)
     S, T, n = w.n_streams, w.n_templates, w.block
     upd = w.updates_per_block()
     nblk = min(w.n_blocks, 16)
@@ -357,6 +358,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--cpu-seconds", type=float, default=12.0, help="target CPU time of one oracle sample")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--time-chunks", type=int, default=0, help="spiir_plan_opts.time_chunks (0 auto, 1 never chunk)")
+    ap.add_argument("--filters", type=int, default=0, help="config 2 only: filters per template of the sweep point")
     ap.add_argument("--graph", default="auto", choices=["auto", "on", "off"],
                     help="replay one captured CUDA graph per step (auto: fall back to eager launches if capture fails)")
     ap.add_argument("--plan-flags", type=int, default=0, help="spiir_plan_opts.flags (bit 0: skip the bank-conflict-avoiding permutation)")

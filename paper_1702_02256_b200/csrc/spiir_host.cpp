@@ -140,7 +140,21 @@ spiir_status compute_geometry(int T, int L, int S, int Dpad, int n, int opt_chun
     const long tasks = (long)S * g->G;
     const long target = (long)n_sm * 8;
     if (opt_chunks >= 1) NC = opt_chunks;
-    else if (tasks * 2 <= target && n >= 128) NC = (int)std::min<long>(target / tasks, n / 64);
+    else if (tasks * 2 <= target && n >= 128) {
+        // Chunking costs two more launches and 1.75x the arithmetic; it pays only when the time a lone
+        // warp needs for the whole block exceeds that.  Cost model from measurements on B200: ~8 us per
+        // launch (window staging, coefficient loads, tail), ~36 ns per time step of a warp, and
+        // proportionally more once more than 4 warps share an SM.
+        const long nc = std::min<long>(target / tasks, n / 64);
+        if (nc >= 2) {
+            const double f0 = 8e-6, tau = 36e-9;
+            const double share_p = std::max(1.0, (double)((tasks + n_sm - 1) / n_sm) / 4.0);
+            const double share_c = std::max(1.0, (double)((tasks * nc + n_sm - 1) / n_sm) / 4.0);
+            const double t_plain = f0 + n * tau * share_p;
+            const double t_chunk = 3.0 * f0 + ((double)n / (double)nc) * tau * 1.75 * share_c;
+            if (t_chunk * 1.15 < t_plain) NC = (int)nc;
+        }
+    }
     NC = std::max(1, std::min(NC, nc_cap));
     int C = round_up((n + NC - 1) / NC, kBatch);
     NC = (n + C - 1) / C;
