@@ -317,6 +317,46 @@ def test_resample_up_and_accumulate(sp, oracle_mod, rows, blocks):
     assert_parity(np.concatenate(zs, -1), np.concatenate(rs, -1), "up2")
 
 
+@pytest.mark.parametrize("n_taps", [32, 64, 192])
+def test_resamplers_other_tap_counts_and_odd_shapes(sp, oracle_mod, n_taps):
+    """32 and 192 taps take the register-blocked kernels (taps in the kernel parameters), 64 the generic
+    ones; shapes that are not multiples of the per-thread blocking (5 inputs up, 10 outputs down)."""
+    import torch
+    rng = np.random.default_rng(n_taps)
+    rows = 37
+    rd, ru = sp.Resampler("down", rows, max_block=3000, n_taps=n_taps), sp.Resampler("up", rows, max_block=1500, n_taps=n_taps)
+    od, ou = oracle_mod.ResampOracle("down", rows, n_taps=n_taps), oracle_mod.ResampOracle("up", rows, n_taps=n_taps)
+    zd, refd, zu, refu = [], [], [], []
+    for n in (2, 46, 2998, 1282, 20):
+        u = rng.standard_normal((rows, n)).astype(np.float32)
+        zd.append(rd.down(torch.from_numpy(u).cuda()).cpu().numpy()); refd.append(od.down(u))
+    for n in (1, 7, 1499, 641, 640, 13):
+        v = (rng.standard_normal((rows, n)) + 1j * rng.standard_normal((rows, n))).astype(np.complex64)
+        base = (rng.standard_normal((rows, 2 * n)) + 1j * rng.standard_normal((rows, 2 * n))).astype(np.complex64)
+        out = torch.from_numpy(base).cuda()
+        ru.up(torch.from_numpy(v).cuda(), out=out, accumulate=True)
+        zu.append(out.cpu().numpy()); refu.append(ou.up(v, out=base.astype(np.complex128)))
+    assert_parity(np.concatenate(zd, -1).astype(np.complex128), np.concatenate(refd, -1).astype(np.complex128), f"down2 N={n_taps}")
+    assert_parity(np.concatenate(zu, -1), np.concatenate(refu, -1), f"up2 N={n_taps}")
+
+
+@pytest.mark.parametrize("n_taps,blocks", [(192, (192, 64, 448)), (32, (256, 128)), (64, (256, 64))])
+def test_multirate_fused_chains_and_fallback(sp, oracle_mod, n_taps, blocks):
+    """192 taps: fused down chain + fused up cascade; 32 taps: fused up cascade, per-stage down kernels;
+    64 taps: one launch per stage both ways.  Ragged block lengths (multiples of 2^(H-1) only)."""
+    w = _inputs().config(3, n_templates=9)
+    banks = [(b.a1, b.b0, b.delays) for b in w.banks]
+    plan = sp.MultiratePlan(banks, [b.rate_hz for b in w.banks], max_block=512, n_taps=n_taps)
+    orc = oracle_mod.MultirateOracle(banks, n_taps=n_taps)
+    rng = np.random.default_rng(n_taps + 1)
+    xs = [rng.standard_normal((1, n)).astype(np.float32) for n in blocks]
+    z = stream_gpu_plan(plan, xs)
+    ref = stream_oracle(orc, xs)
+    assert_parity(z, ref, f"multirate N={n_taps}")
+    expect = {192: 2, 32: 1 + 6, 64: 12}[n_taps]
+    assert plan.launches(256) >= expect
+
+
 def test_kaiser_taps_match_oracle_design(sp, oracle_mod):
     """The library generates its own taps (no shared table); they agree with the oracle's to 1 ulp."""
     h = sp.spiir_kaiser_taps(192, 5.0, 0.25)
