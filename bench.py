@@ -40,6 +40,10 @@ METRIC = "SPIIR filter-sample updates/s (templates*filters*samples/s)"
 UNIT = "updates/s"
 FLOP_PER_UPDATE = 12
 FP32_LANES_PER_SM = 128         # B200 SM: 4 sub-partitions x 32 FP32 lanes (guides/B300_MICROARCH.md)
+# dram__bytes_read.sum + dram__bytes_write.sum of one spiir_filter_kernel launch, from the committed
+# `ncu --set full` captures (profiles/r1c_summary.md); per launch, like roofline.achieved
+NCU_DRAM_TRAFFIC = {"cfg1_many_filter_1024x256": 7.428352e6 + 0.137472e6,
+                    "cfg4_full_bank_2x16384x256": 235.036672e6 + 556.152064e6}
 
 
 def _dist_env():
@@ -309,7 +313,7 @@ def bench_ours(args):
         peak_tflops = props.multi_processor_count * FP32_LANES_PER_SM * 2 * sm_max_mhz * 1e6 / 1e12
         achieved = FLOP_PER_UPDATE * upd / (ms_per_step * 1e-3) / 1e12
         roofline = {"bound": "alu", "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s",
-                    "frac": achieved / peak_tflops, "traffic": None,
+                    "frac": achieved / peak_tflops, "traffic": NCU_DRAM_TRAFFIC.get(w.name),
                     "kernel": "spiir_filter_kernel" if len(w.banks) == 1 else "spiir_filter_kernel + resamplers (whole step)",
                     "peak_source": f"derived: {props.multi_processor_count} SMs x {FP32_LANES_PER_SM} FP32 lanes x 2 flop x "
                                    f"{sm_max_mhz:.0f} MHz (clocks.max.sm, MEASURED_PEAKS.json); 12 flop per update (PAPER.md:88)"}
@@ -349,6 +353,66 @@ def bench_ours(args):
     return 0
 
 
+def bench_resample(args):
+    """Standalone x2 stage (spiir_resample_up with accumulate / spiir_resample_down) on a batch large enough
+    to leave the launch-bound regime: rows = 16384, 2048 -> 4096 (up) or 4096 -> 2048 (down), 192 taps.
+    Reports both rooflines DESIGN.md discusses: HBM (algorithmic bytes per output) and FP32 FMA."""
+    import torch
+    import paper_1702_02256_b200 as sp
+    sp.lib()
+    torch.cuda.set_device(0)
+    up = args.resample == "up"
+    rows, n_in, taps = args.rows, (2048 if up else 4096), 192
+    r = sp.Resampler("up" if up else "down", rows, max_block=n_in, n_taps=taps)
+    if up:
+        v = torch.randn(rows, n_in, dtype=torch.complex64, device="cuda")
+        out = torch.zeros(rows, 2 * n_in, dtype=torch.complex64, device="cuda")
+        call = lambda: r.up(v, out, accumulate=True)
+        n_out, bytes_per_out, fma_per_out = rows * 2 * n_in, 20.0, taps            # 4 in + 8 read + 8 written; 96 taps x (re, im)
+    else:
+        u = torch.randn(rows, n_in, dtype=torch.float32, device="cuda")
+        out = torch.zeros(rows, n_in // 2, dtype=torch.float32, device="cuda")
+        call = lambda: r.down(u, out)
+        n_out, bytes_per_out, fma_per_out = rows * n_in // 2, 12.0, taps           # 8 in + 4 written; 192 taps
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+    stream = torch.cuda.current_stream()
+    for _ in range(max(3, args.warmup)):
+        call()
+    torch.cuda.synchronize()
+    sampler = ClockSampler(0); sampler.start()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    for i in range(args.steps):
+        flush.fill_(i & 0xFF)
+        ev[i][0].record(stream); call(); ev[i][1].record(stream)
+    torch.cuda.synchronize()
+    clocks = sampler.stop()
+    ms = float(np.mean([a.elapsed_time(b) for a, b in ev]))
+    peaks = {}
+    try:
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:
+        pass
+    hbm_peak = float(peaks.get("hbm_gbs") or 6542.7)
+    props = torch.cuda.get_device_properties(0)
+    sm_max_mhz = float(peaks.get("sm_max_mhz") or clocks.get("sm_max_mhz") or 1965.0)
+    fma_peak = props.multi_processor_count * FP32_LANES_PER_SM * sm_max_mhz * 1e6           # FMA lane-ops per second
+    gbs = n_out * bytes_per_out / (ms * 1e-3) / 1e9
+    line = {"metric": f"x2 resampler ({args.resample}) output samples/s", "value": n_out / (ms * 1e-3), "unit": "samples/s",
+            "n_gpus": 1, "steps": args.steps, "warmup": max(3, args.warmup), "ms_per_step": ms, "higher_is_better": True,
+            "dtype": "f32", "data": "synthetic",
+            "config": {"workload": f"resample_{args.resample}_{rows}x{n_in}_{taps}taps", "rows": rows, "n_in": n_in, "n_taps": taps,
+                       "l2": "flushed between timed steps (256 MiB write)"},
+            "clocks": clocks, "gpu_launches": args.steps,
+            "roofline": {"bound": "alu", "achieved": n_out * fma_per_out * 2 / (ms * 1e-3) / 1e12, "peak": 2 * fma_peak / 1e12,
+                         "unit": "TFLOP/s", "frac": n_out * fma_per_out / (ms * 1e-3) / fma_peak, "traffic": None,
+                         "kernel": "spiir_up2_fir_kernel<96>" if up else "spiir_down2_fir_kernel<192>",
+                         "note": "192 FMA per output sample: FP32-bound, not HBM-bound (DESIGN.md 5.2)"},
+            "roofline_hbm": {"bound": "hbm", "achieved": gbs, "peak": hbm_peak, "unit": "GB/s", "frac": gbs / hbm_peak,
+                             "bytes_per_output": bytes_per_out}}
+    print(json.dumps(line), flush=True)
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -360,12 +424,17 @@ def main():
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--time-chunks", type=int, default=0, help="spiir_plan_opts.time_chunks (0 auto, 1 never chunk)")
     ap.add_argument("--filters", type=int, default=0, help="config 2 only: filters per template of the sweep point")
+    ap.add_argument("--resample", default="", choices=["", "up", "down"],
+                    help="time the exported x2 stage alone (rows x 2048 -> 4096 up+accumulate, or rows x 4096 -> 2048 down)")
+    ap.add_argument("--rows", type=int, default=16384, help="rows of the --resample batch")
     ap.add_argument("--graph", default="auto", choices=["auto", "on", "off"],
                     help="replay one captured CUDA graph per step (auto: fall back to eager launches if capture fails)")
     ap.add_argument("--plan-flags", type=int, default=0, help="spiir_plan_opts.flags (bit 0: skip the bank-conflict-avoiding permutation)")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3
+    if args.resample:
+        return bench_resample(args)
     if args.impl == "reference":
         return bench_reference(args)
     return bench_ours(args)

@@ -20,6 +20,10 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#ifndef SPIIR_STAMP
+#define SPIIR_STAMP(i)
+#endif
+
 namespace spiir {
 
 constexpr int kBatch = 16;        // time steps per reduction batch
@@ -32,7 +36,7 @@ struct FilterArgs {
     float2*       chunk_st;  // chunked modes: [S][NC][G][F][32]; pass 1 writes end states, carry
                              // turns them into initial states in place, pass 2 reads them
     float*        hbuf[2];   // [S][Dpad] input history, ping-pong: hbuf[phase] holds the Dpad samples before
-                             // this block (oldest first), hbuf[phase ^ 1] is written by CTA (0, s, chunk 0)
+                             // this block (oldest first), hbuf[phase ^ 1] is written in slices by the CTAs of stream s
     int*          phase;     // device words {phase, arrivals}: which buffer is current is decided on the
                              // device, so that every call enqueues identical work (CUDA-graph replayable)
     const float*  x;         // [S][n]
@@ -256,6 +260,7 @@ __global__ void __launch_bounds__(kMaxWarps * 32) spiir_filter_kernel(const Filt
     const int s = blockIdx.y / a.NC, c = blockIdx.y % a.NC;
     const int tc0 = c * a.C;                                            // chunk range [tc0, tc1)
     const int tc1 = min(a.n, tc0 + a.C);
+    SPIIR_STAMP(0);
     const int ph = phase_read(a.phase);
     const float* hist_s = a.hbuf[ph] + (size_t)s * a.Dpad;
     const float* x_s = a.x + (size_t)s * a.n;
@@ -263,17 +268,22 @@ __global__ void __launch_bounds__(kMaxWarps * 32) spiir_filter_kernel(const Filt
     if (threadIdx.x == 0) mbar_init(bar, 1);
     __syncthreads();
 
-    // carried history for the next block (reads only hist + x: no race with other CTAs)
-    if (a.mode != 1 && blockIdx.x == 0 && c == 0) {
+    // carried history for the next block (reads only hist + x: no race with other CTAs).  Every CTA of the
+    // stream copies a slice: one CTA doing all Dpad samples is a chain of ~Dpad/blockDim dependent global
+    // round trips (11 us for 4096 samples) that the whole launch then waits for.
+    if (a.mode != 1) {
         float* hn = a.hbuf[ph ^ 1] + (size_t)s * a.Dpad;
-        for (int i = threadIdx.x; i < a.Dpad; i += blockDim.x) {
+        const int cta = c * gridDim.x + blockIdx.x, nctas = a.NC * gridDim.x;
+        for (int i = cta * blockDim.x + threadIdx.x; i < a.Dpad; i += nctas * blockDim.x) {
             int g = a.n - a.Dpad + i;
             hn[i] = (g >= 0) ? x_s[g] : hist_s[a.n + i];
         }
     }
 
+    SPIIR_STAMP(1);
     const int ntiles = (tc1 - tc0 + a.NT - 1) / a.NT;
     if (ntiles == 1) stage_window(win, bar, parity, a, hist_s, x_s, tc0);
+    SPIIR_STAMP(2);
     const float4* win4 = reinterpret_cast<const float4*>(win);
 
     constexpr int TPG = 32 / LPT;                                       // templates per group
@@ -300,6 +310,7 @@ __global__ void __launch_bounds__(kMaxWarps * 32) spiir_filter_kernel(const Filt
             Y[f] = y0;
         }
         float2* zt = active ? a.z + ((size_t)s * a.T + t) * (size_t)a.n : nullptr;
+        SPIIR_STAMP(3);
 
         for (int tile = 0; tile < ntiles; ++tile) {
             const int t0 = tc0 + tile * a.NT;
@@ -317,6 +328,7 @@ __global__ void __launch_bounds__(kMaxWarps * 32) spiir_filter_kernel(const Filt
                 if (!NOZ) reduce_store<LPT>(Z, lane, zt + t0 + nfull * kBatch, rem, active, a.accumulate != 0);
             }
         }
+        SPIIR_STAMP(4);
         if (wactive) {
 #pragma unroll
             for (int f = 0; f < F; ++f) {
@@ -328,6 +340,7 @@ __global__ void __launch_bounds__(kMaxWarps * 32) spiir_filter_kernel(const Filt
         }
     }
     if (a.mode != 1 && last_cta_arrives(a.phase, gridDim.x * gridDim.y)) a.phase[0] = ph ^ 1;
+    SPIIR_STAMP(5);
 }
 
 // ---------------------------------------------------------------------------------------------
