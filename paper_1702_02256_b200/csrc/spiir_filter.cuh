@@ -20,10 +20,6 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
-#ifndef SPIIR_STAMP
-#define SPIIR_STAMP(i)
-#endif
-
 namespace spiir {
 
 constexpr int kBatch = 16;        // time steps per reduction batch
@@ -260,7 +256,6 @@ __global__ void __launch_bounds__(kMaxWarps * 32) spiir_filter_kernel(const Filt
     const int s = blockIdx.y / a.NC, c = blockIdx.y % a.NC;
     const int tc0 = c * a.C;                                            // chunk range [tc0, tc1)
     const int tc1 = min(a.n, tc0 + a.C);
-    SPIIR_STAMP(0);
     const int ph = phase_read(a.phase);
     const float* hist_s = a.hbuf[ph] + (size_t)s * a.Dpad;
     const float* x_s = a.x + (size_t)s * a.n;
@@ -279,11 +274,8 @@ __global__ void __launch_bounds__(kMaxWarps * 32) spiir_filter_kernel(const Filt
             hn[i] = (g >= 0) ? x_s[g] : hist_s[a.n + i];
         }
     }
-
-    SPIIR_STAMP(1);
     const int ntiles = (tc1 - tc0 + a.NT - 1) / a.NT;
     if (ntiles == 1) stage_window(win, bar, parity, a, hist_s, x_s, tc0);
-    SPIIR_STAMP(2);
     const float4* win4 = reinterpret_cast<const float4*>(win);
 
     constexpr int TPG = 32 / LPT;                                       // templates per group
@@ -310,7 +302,6 @@ __global__ void __launch_bounds__(kMaxWarps * 32) spiir_filter_kernel(const Filt
             Y[f] = y0;
         }
         float2* zt = active ? a.z + ((size_t)s * a.T + t) * (size_t)a.n : nullptr;
-        SPIIR_STAMP(3);
 
         for (int tile = 0; tile < ntiles; ++tile) {
             const int t0 = tc0 + tile * a.NT;
@@ -328,7 +319,6 @@ __global__ void __launch_bounds__(kMaxWarps * 32) spiir_filter_kernel(const Filt
                 if (!NOZ) reduce_store<LPT>(Z, lane, zt + t0 + nfull * kBatch, rem, active, a.accumulate != 0);
             }
         }
-        SPIIR_STAMP(4);
         if (wactive) {
 #pragma unroll
             for (int f = 0; f < F; ++f) {
@@ -340,7 +330,6 @@ __global__ void __launch_bounds__(kMaxWarps * 32) spiir_filter_kernel(const Filt
         }
     }
     if (a.mode != 1 && last_cta_arrives(a.phase, gridDim.x * gridDim.y)) a.phase[0] = ph ^ 1;
-    SPIIR_STAMP(5);
 }
 
 // ---------------------------------------------------------------------------------------------
