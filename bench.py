@@ -362,18 +362,18 @@ def bench_resample(args):
     sp.lib()
     torch.cuda.set_device(0)
     up = args.resample == "up"
-    rows, n_in, taps = args.rows, (2048 if up else 4096), 192
+    rows, n_in, taps = args.rows, (2048 if up else 4096), args.taps
     r = sp.Resampler("up" if up else "down", rows, max_block=n_in, n_taps=taps)
     if up:
         v = torch.randn(rows, n_in, dtype=torch.complex64, device="cuda")
         out = torch.zeros(rows, 2 * n_in, dtype=torch.complex64, device="cuda")
         call = lambda: r.up(v, out, accumulate=True)
-        n_out, bytes_per_out, fma_per_out = rows * 2 * n_in, 20.0, taps            # 4 in + 8 read + 8 written; 96 taps x (re, im)
+        n_out, bytes_per_out, fma_per_out = rows * 2 * n_in, 20.0, taps            # 4 in + 8 read + 8 written; taps/2 x (re, im)
     else:
         u = torch.randn(rows, n_in, dtype=torch.float32, device="cuda")
         out = torch.zeros(rows, n_in // 2, dtype=torch.float32, device="cuda")
         call = lambda: r.down(u, out)
-        n_out, bytes_per_out, fma_per_out = rows * n_in // 2, 12.0, taps           # 8 in + 4 written; 192 taps
+        n_out, bytes_per_out, fma_per_out = rows * n_in // 2, 12.0, taps           # 8 in + 4 written; one FMA per tap
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
     stream = torch.cuda.current_stream()
     for _ in range(max(3, args.warmup)):
@@ -405,8 +405,8 @@ def bench_resample(args):
             "clocks": clocks, "gpu_launches": args.steps,
             "roofline": {"bound": "alu", "achieved": n_out * fma_per_out * 2 / (ms * 1e-3) / 1e12, "peak": 2 * fma_peak / 1e12,
                          "unit": "TFLOP/s", "frac": n_out * fma_per_out / (ms * 1e-3) / fma_peak, "traffic": None,
-                         "kernel": "spiir_up2_fir_kernel<96>" if up else "spiir_down2_fir_kernel<192>",
-                         "note": "192 FMA per output sample: FP32-bound, not HBM-bound (DESIGN.md 5.2)"},
+                         "kernel": f"spiir_up2_fir_kernel<{taps // 2}>" if up else f"spiir_down2_fir_kernel<{taps}>",
+                         "note": f"{taps} FMA per output sample (DESIGN.md 5.2: 192 taps are FP32-bound, 32 taps HBM-bound)"},
             "roofline_hbm": {"bound": "hbm", "achieved": gbs, "peak": hbm_peak, "unit": "GB/s", "frac": gbs / hbm_peak,
                              "bytes_per_output": bytes_per_out}}
     print(json.dumps(line), flush=True)
@@ -427,6 +427,8 @@ def main():
     ap.add_argument("--resample", default="", choices=["", "up", "down"],
                     help="time the exported x2 stage alone (rows x 2048 -> 4096 up+accumulate, or rows x 4096 -> 2048 down)")
     ap.add_argument("--rows", type=int, default=16384, help="rows of the --resample batch")
+    ap.add_argument("--taps", type=int, default=192, choices=[32, 192],
+                    help="FIR length of the --resample stage (192: configs[3]; 32: the paper's own up-filter, PAPER.md:88)")
     ap.add_argument("--graph", default="auto", choices=["auto", "on", "off"],
                     help="replay one captured CUDA graph per step (auto: fall back to eager launches if capture fails)")
     ap.add_argument("--plan-flags", type=int, default=0, help="spiir_plan_opts.flags (bit 0: skip the bank-conflict-avoiding permutation)")

@@ -184,6 +184,22 @@ __global__ void __launch_bounds__(128, 8) spiir_up2_fir_kernel(const UpArgs a, c
     const float2* hcur = a.hbuf[ph];
     float2* hnext = a.hbuf[ph ^ 1];
 
+    // Short filters (32 taps) are HBM-bound: the tile of `out` that is accumulated into is then fetched with
+    // cp.async while the inputs are staged and the FIR runs, and added in shared memory (PREFETCH).  With
+    // 192 taps the FIR hides that read anyway and the extra pass only costs issue slots.
+    constexpr bool PREFETCH = HALF <= 16;
+    const bool pre = PREFETCH && a.accumulate != 0;
+    if (pre) {
+        for (int sl = 0; sl < nrow; ++sl) {
+            const float2* src = a.out + (size_t)(row0 + sl) * 2 * a.n_in + 2 * m_base;
+            float2* dst = vout + (size_t)sl * out_stride;
+            for (int i = threadIdx.x; i < seg_len; i += blockDim.x) {
+                const uint32_t d = (uint32_t)__cvta_generic_to_shared(dst + 2 * i);
+                asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(src + 2 * i) : "memory");
+            }
+        }
+        asm volatile("cp.async.commit_group;" ::: "memory");
+    }
     // stage inputs: vin[slot][i] = v[row][m_base - H + i], i in [0, seg_len + H); zero beyond
 #pragma unroll 4
     for (int sl = 0; sl < nrow; ++sl) {
@@ -203,12 +219,13 @@ __global__ void __launch_bounds__(128, 8) spiir_up2_fir_kernel(const UpArgs a, c
     __syncthreads();
 
     const int slot = threadIdx.x / a.upr, unit = threadIdx.x % a.upr;
-    if (slot < nrow && unit * R < seg_len) {
+    const bool live = slot < nrow && unit * R < seg_len;
+    float2 acc0[R], acc1[R];
+#pragma unroll
+    for (int r = 0; r < R; ++r) { acc0[r] = make_float2(0.f, 0.f); acc1[r] = make_float2(0.f, 0.f); }
+    if (live) {
         // inputs of this thread: local indices [unit*R, unit*R + R + H), newest = unit*R + R - 1 + H
         const float2* vp = vin + (size_t)slot * in_stride + unit * R;
-        float2 acc0[R], acc1[R];
-#pragma unroll
-        for (int r = 0; r < R; ++r) { acc0[r] = make_float2(0.f, 0.f); acc1[r] = make_float2(0.f, 0.f); }
 #pragma unroll
         for (int jj = 0; jj < R + H; ++jj) {
             const float2 v = vp[R - 1 + H - jj];                        // input i = m0 + R - 1 - jj
@@ -223,11 +240,22 @@ __global__ void __launch_bounds__(128, 8) spiir_up2_fir_kernel(const UpArgs a, c
                 }
             }
         }
+    }
+    if (pre) {                                                          // every thread's cp.async has landed
+        asm volatile("cp.async.wait_group 0;" ::: "memory");
+        __syncthreads();
+    }
+    if (live) {
         float2* op = vout + (size_t)slot * out_stride + 2 * unit * R;
 #pragma unroll
         for (int r = 0; r < R; ++r) {
-            op[2 * r] = make_float2(2.f * acc0[r].x, 2.f * acc0[r].y);
-            op[2 * r + 1] = make_float2(2.f * acc1[r].x, 2.f * acc1[r].y);
+            float2 w0 = make_float2(2.f * acc0[r].x, 2.f * acc0[r].y), w1 = make_float2(2.f * acc1[r].x, 2.f * acc1[r].y);
+            if (pre && unit * R + r < seg_len) {
+                const float2 p0 = op[2 * r], p1 = op[2 * r + 1];
+                w0.x += p0.x; w0.y += p0.y; w1.x += p1.x; w1.y += p1.y;
+            }
+            op[2 * r] = w0;
+            op[2 * r + 1] = w1;
         }
     }
     __syncthreads();
@@ -239,7 +267,7 @@ __global__ void __launch_bounds__(128, 8) spiir_up2_fir_kernel(const UpArgs a, c
         const float4* src = reinterpret_cast<const float4*>(vout + (size_t)sl * out_stride);
         for (int i = threadIdx.x; i < seg_len; i += blockDim.x) {
             float4 w = src[i];
-            if (a.accumulate) { const float4 p = o[i]; w.x += p.x; w.y += p.y; w.z += p.z; w.w += p.w; }
+            if (a.accumulate && !pre) { const float4 p = o[i]; w.x += p.x; w.y += p.y; w.z += p.z; w.w += p.w; }
             o[i] = w;
         }
     }
