@@ -78,6 +78,17 @@ static filter_kernel_t pick_kernel(int F, int LPT, bool noz)
         case 2: return pick_small<2>(F, noz);
         case 4: return pick_small<4>(F, noz);
         case 8: return pick_small<8>(F, noz);
+        case 16:
+            switch (F) {
+                case 2: return pick_noz<2, 16>(noz);
+                case 3: return pick_noz<3, 16>(noz);
+                case 4: return pick_noz<4, 16>(noz);
+                case 5: return pick_noz<5, 16>(noz);
+                case 6: return pick_noz<6, 16>(noz);
+                case 7: return pick_noz<7, 16>(noz);
+                case 8: return pick_noz<8, 16>(noz);
+            }
+            return nullptr;
         case 32:
             switch (F) {
                 case 1: return pick_noz<1, 32>(noz);
@@ -168,7 +179,7 @@ spiir_status spiir_plan_create(spiir_plan_t** out, const spiir_c64* a1, const sp
         dmax = std::max(dmax, (int)delays[i]);
     }
     int F, LPT;
-    if (!choose_lane_mapping(n_filters, &F, &LPT)) {
+    if (!choose_lane_mapping(n_filters, n_templates, &F, &LPT)) {
         set_error("spiir_plan_create: n_filters = %d not supported (1..512)", n_filters);
         return SPIIR_EUNSUPPORTED;
     }

@@ -4,6 +4,7 @@
 #include <math.h>
 #include <stdarg.h>
 #include <stdio.h>
+#include <stdlib.h>
 #include <string.h>
 
 #include <algorithm>
@@ -30,9 +31,13 @@ const char* last_error() { return g_err; }
 //   32..512       : the 32 lanes of a warp, F = ceil(L/32) rounded up to an instantiated F
 static const int kFWarp[] = {1, 2, 3, 4, 5, 6, 7, 8, 10, 12, 14, 16};
 
-bool choose_lane_mapping(int L, int* F, int* LPT)
+bool choose_lane_mapping(int L, int T, int* F, int* LPT)
 {
     if (L < 1) return false;
+    // 32..128 filters and enough templates to give every SM several warps anyway: half a warp per template
+    // (two templates per warp).  The 16 outputs of a batch then cost a 16-lane butterfly for TWO templates,
+    // i.e. half the shuffle / select work per update of the one-warp-per-template mapping.
+    if (L >= 32 && L <= 128 && T >= lpt16_min_templates()) { *LPT = 16; *F = (L + 15) / 16; return true; }
     if (L <= 4) { *LPT = 1; *F = L; return true; }
     if (L <= 8) { *LPT = 2; *F = (L + 1) / 2; return true; }
     if (L <= 16) { *LPT = 4; *F = (L + 3) / 4; return true; }
@@ -41,6 +46,13 @@ bool choose_lane_mapping(int L, int* F, int* LPT)
     for (int f : kFWarp)
         if (f >= need) { *LPT = 32; *F = f; return true; }
     return false;
+}
+
+int lpt16_min_templates()
+{
+    // measured on B200 (148 SMs): with 4096 templates the half-warp mapping is 10-30 % faster for 32..128
+    // filters, with 1024 templates (3.5 warps per SM left) it is not; switch where >= 8 warps per SM remain
+    return 16 * 148;
 }
 
 static inline int bank_class(int d) { return ((d + 3) >> 2) & 7; }   // 16-byte bank group of W[Dpad + j - d]
@@ -128,7 +140,7 @@ spiir_status compute_geometry(int T, int L, int S, int Dpad, int n, int opt_chun
                               int smem_optin, FilterGeometry* g)
 {
     memset(g, 0, sizeof *g);
-    if (!choose_lane_mapping(L, &g->F, &g->LPT)) {
+    if (!choose_lane_mapping(L, T, &g->F, &g->LPT)) {
         set_error("n_filters = %d is not supported (1..512)", L);
         return SPIIR_EUNSUPPORTED;
     }
@@ -238,7 +250,7 @@ spiir_status spiir_host_layout(const spiir_c64* a1, const spiir_c64* b0, const i
                                int32_t* dly_out, int info[4], double* conflict_degree)
 {
     int F, LPT;
-    if (!a1 || !b0 || !delays || n_templates < 1 || !spiir::choose_lane_mapping(n_filters, &F, &LPT)) {
+    if (!a1 || !b0 || !delays || n_templates < 1 || !spiir::choose_lane_mapping(n_filters, n_templates, &F, &LPT)) {
         spiir::set_error("spiir_host_layout: bad arguments");
         return SPIIR_EINVAL;
     }

@@ -36,7 +36,8 @@ struct FilterGeometry {
 };
 
 // Pick (F, LPT) for a bank of L filters per template.  Returns false when L is not supported.
-bool choose_lane_mapping(int L, int* F, int* LPT);
+bool choose_lane_mapping(int L, int T, int* F, int* LPT);
+int lpt16_min_templates();
 
 // Position (index into the [G][F][32] plan arrays) of every filter [T][L]; fills the permuted
 // coefficient / delay arrays (zero padded).  avoid_conflicts: spread the 16-byte bank groups of

@@ -82,6 +82,22 @@ def test_config1_full_size_sampled(sp, oracle_mod):
     assert_parity(z[:, idx], ref, "cfg1 full sampled")
 
 
+def test_half_warp_per_template_mapping(sp, oracle_mod):
+    """Banks of 32..128 filters with >= 2368 templates put two templates in a warp (16 lanes each)."""
+    for L in (40, 128):
+        w = _inputs().config(1, n_templates=2400, n_filters=L)
+        b = w.banks[0]
+        plan = sp.Plan(b.a1, b.b0, b.delays % 300, b.rate_hz, max_block=256)
+        info = plan.launch_info(256)
+        assert info["lanes_per_template"] == 16 and info["F"] == (L + 15) // 16
+        rng = np.random.default_rng(L)
+        xs = [rng.standard_normal((1, n)).astype(np.float32) for n in (256, 37, 160)]
+        z = stream_gpu_plan(plan, xs)
+        idx = np.array([0, 1, 2, 3, 1199, 1200, 2397, 2398, 2399])
+        ref = stream_oracle(oracle_mod.FilterOracle(b.a1[idx], b.b0[idx], (b.delays % 300)[idx]), xs)
+        assert_parity(z[:, idx], ref, f"LPT16 L={L}")
+
+
 # ------------------------------------------------------------------------------------------------
 # config 2: few-filter sweep, 4096 templates, 256-sample blocks
 # ------------------------------------------------------------------------------------------------

@@ -83,6 +83,16 @@ def test_lane_mapping(sp, L, F, LPT):
     assert F * LPT >= L
 
 
+def test_lane_mapping_many_templates(sp):
+    # 32..128 filters and at least 16 x 148 templates: two templates per warp, 16 lanes each
+    g = sp.spiir_host_geometry(4096, 64, 1, 100, 1024)
+    assert (g["F"], g["lanes_per_template"]) == (4, 16)
+    g = sp.spiir_host_geometry(4096, 129, 1, 100, 1024)
+    assert (g["F"], g["lanes_per_template"]) == (5, 32)
+    g = sp.spiir_host_geometry(2367, 64, 1, 100, 1024)
+    assert (g["F"], g["lanes_per_template"]) == (2, 32)
+
+
 def test_layout_is_a_permutation_and_avoids_bank_conflicts(sp):
     from paper_1702_02256_b200 import inputs
     b = inputs.config(1, n_templates=16).banks[0]
