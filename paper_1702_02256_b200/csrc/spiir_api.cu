@@ -113,19 +113,26 @@ spiir_status plan_geometry(const spiir_plan* p, int n, FilterGeometry* g)
     return compute_geometry(p->T, p->L, p->S, p->Dpad, n, p->opt_chunks, p->NC_cap, p->dev.n_sm, p->dev.smem_optin, g);
 }
 
+static void fill_filter_args(const spiir_plan* p, const float* x, int n, spiir_c64* z, int accumulate, const FilterGeometry& g,
+                             FilterArgs* a)
+{
+    a->coef = p->d_coef; a->dly = p->d_dly; a->state = p->d_state; a->chunk_st = p->d_chunk;
+    a->hbuf[0] = p->d_hist[0]; a->hbuf[1] = p->d_hist[1]; a->phase = p->d_phase;
+    a->x = x; a->z = reinterpret_cast<float2*>(z);
+    a->n = n; a->T = p->T; a->G = p->G; a->S = p->S; a->Dpad = p->Dpad;
+    a->NT = g.NT; a->CS = g.CS; a->NC = g.NC; a->C = g.C;
+    a->x_aligned = ((reinterpret_cast<uintptr_t>(x) & 15u) == 0 && (p->S == 1 || (n & 3) == 0)) ? 1 : 0;
+    a->accumulate = accumulate;
+    a->mode = 0;
+}
+
 spiir_status filter_launch(spiir_plan* p, const float* x, int n, spiir_c64* z, int accumulate, cudaStream_t st)
 {
     FilterGeometry g;
     spiir_status rc = plan_geometry(p, n, &g);
     if (rc != SPIIR_OK) return rc;
     FilterArgs a;
-    a.coef = p->d_coef; a.dly = p->d_dly; a.state = p->d_state; a.chunk_st = p->d_chunk;
-    a.hbuf[0] = p->d_hist[0]; a.hbuf[1] = p->d_hist[1]; a.phase = p->d_phase;
-    a.x = x; a.z = reinterpret_cast<float2*>(z);
-    a.n = n; a.T = p->T; a.G = p->G; a.S = p->S; a.Dpad = p->Dpad;
-    a.NT = g.NT; a.CS = g.CS; a.NC = g.NC; a.C = g.C;
-    a.x_aligned = ((reinterpret_cast<uintptr_t>(x) & 15u) == 0 && (p->S == 1 || (n & 3) == 0)) ? 1 : 0;
-    a.accumulate = accumulate;
+    fill_filter_args(p, x, n, z, accumulate, g, &a);
     const dim3 grid(g.grid_x, g.grid_y), block(g.warps * 32);
     for (int pass = 0; pass < (g.NC > 1 ? 2 : 1); ++pass) {
         a.mode = g.NC > 1 ? pass + 1 : 0;
@@ -140,6 +147,51 @@ spiir_status filter_launch(spiir_plan* p, const float* x, int n, spiir_c64* z, i
             SPIIR_CUDA(cudaGetLastError());
         }
     }
+    return SPIIR_OK;
+}
+
+// Several unchunked banks with the same lane mapping in ONE launch (blockIdx.z = bank).  Returns
+// SPIIR_EUNSUPPORTED when the banks do not qualify; the caller then launches them one by one.
+typedef void (*multi_kernel_t)(const MultiFilterArgs);
+static multi_kernel_t pick_multi(int F, int LPT)
+{
+    if (LPT != 32) return nullptr;
+    switch (F) {
+        case 1: return spiir_filter_multi_kernel<1, 32>;
+        case 2: return spiir_filter_multi_kernel<2, 32>;
+        case 3: return spiir_filter_multi_kernel<3, 32>;
+        case 4: return spiir_filter_multi_kernel<4, 32>;
+        case 5: return spiir_filter_multi_kernel<5, 32>;
+        case 6: return spiir_filter_multi_kernel<6, 32>;
+        case 7: return spiir_filter_multi_kernel<7, 32>;
+        case 8: return spiir_filter_multi_kernel<8, 32>;
+    }
+    return nullptr;
+}
+
+spiir_status filter_launch_group(spiir_plan* const* ps, const float* const* xs, const int* ns, spiir_c64* const* zs, int count,
+                                 cudaStream_t st)
+{
+    if (count < 2 || count > kMaxMulti) return SPIIR_EUNSUPPORTED;
+    MultiFilterArgs m;
+    int F = 0, LPT = 0, warps = 0, gx = 0, gy = 0, smem = 0;
+    for (int k = 0; k < count; ++k) {
+        FilterGeometry g;
+        spiir_status rc = plan_geometry(ps[k], ns[k], &g);
+        if (rc != SPIIR_OK) return rc;
+        if (g.NC != 1) return SPIIR_EUNSUPPORTED;
+        if (k == 0) { F = g.F; LPT = g.LPT; }
+        else if (g.F != F || g.LPT != LPT) return SPIIR_EUNSUPPORTED;
+        fill_filter_args(ps[k], xs[k], ns[k], zs[k], 0, g, &m.bank[k]);
+        m.gx[k] = g.grid_x; m.gy[k] = g.grid_y;
+        warps = std::max(warps, g.warps); gx = std::max(gx, g.grid_x); gy = std::max(gy, g.grid_y);
+        smem = std::max(smem, g.smem_bytes);
+    }
+    multi_kernel_t k = pick_multi(F, LPT);
+    if (!k) return SPIIR_EUNSUPPORTED;
+    SPIIR_CUDA(ensure_smem((const void*)k, smem));
+    k<<<dim3(gx, gy, count), warps * 32, smem, st>>>(m);
+    SPIIR_CUDA(cudaGetLastError());
     return SPIIR_OK;
 }
 

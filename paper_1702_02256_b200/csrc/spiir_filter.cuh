@@ -245,15 +245,17 @@ __device__ __forceinline__ void batch_steps(const float4* __restrict__ win4, con
     }
 }
 
+// The kernel body takes its CTA coordinates as arguments so that one launch can also serve several banks
+// (spiir_filter_multi_kernel below): bx in [0, gdx), by in [0, gdy) with gdy = S * NC.
 template <int F, int LPT, bool NOZ>
-__global__ void __launch_bounds__(kMaxWarps * 32) spiir_filter_kernel(const FilterArgs a)
+__device__ __forceinline__ void filter_body(const FilterArgs& a, const int bx, const int by, const int gdx, const int gdy)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     float* win = reinterpret_cast<float*>(smem_raw);                   // 4 copies x CS floats
     uint64_t* bar = reinterpret_cast<uint64_t*>(win + 4 * (size_t)a.CS);
 
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
-    const int s = blockIdx.y / a.NC, c = blockIdx.y % a.NC;
+    const int s = by / a.NC, c = by % a.NC;
     const int tc0 = c * a.C;                                            // chunk range [tc0, tc1)
     const int tc1 = min(a.n, tc0 + a.C);
     const int ph = phase_read(a.phase);
@@ -268,7 +270,7 @@ __global__ void __launch_bounds__(kMaxWarps * 32) spiir_filter_kernel(const Filt
     // round trips (11 us for 4096 samples) that the whole launch then waits for.
     if (a.mode != 1) {
         float* hn = a.hbuf[ph ^ 1] + (size_t)s * a.Dpad;
-        const int cta = c * gridDim.x + blockIdx.x, nctas = a.NC * gridDim.x;
+        const int cta = c * gdx + bx, nctas = a.NC * gdx;
         for (int i = cta * blockDim.x + threadIdx.x; i < a.Dpad; i += nctas * blockDim.x) {
             int g = a.n - a.Dpad + i;
             hn[i] = (g >= 0) ? x_s[g] : hist_s[a.n + i];
@@ -279,7 +281,7 @@ __global__ void __launch_bounds__(kMaxWarps * 32) spiir_filter_kernel(const Filt
     const float4* win4 = reinterpret_cast<const float4*>(win);
 
     constexpr int TPG = 32 / LPT;                                       // templates per group
-    for (int g0 = blockIdx.x * nwarps; g0 < a.G; g0 += gridDim.x * nwarps) {
+    for (int g0 = bx * nwarps; g0 < a.G; g0 += gdx * nwarps) {
         const int g = g0 + warp;
         const bool wactive = g < a.G;
         const int t = g * TPG + lane / LPT;
@@ -329,7 +331,29 @@ __global__ void __launch_bounds__(kMaxWarps * 32) spiir_filter_kernel(const Filt
             }
         }
     }
-    if (a.mode != 1 && last_cta_arrives(a.phase, gridDim.x * gridDim.y)) a.phase[0] = ph ^ 1;
+    if (a.mode != 1 && last_cta_arrives(a.phase, gdx * gdy)) a.phase[0] = ph ^ 1;
+}
+
+template <int F, int LPT, bool NOZ>
+__global__ void __launch_bounds__(kMaxWarps * 32) spiir_filter_kernel(const FilterArgs a)
+{
+    filter_body<F, LPT, NOZ>(a, blockIdx.x, blockIdx.y, gridDim.x, gridDim.y);
+}
+
+// Several banks that share a lane mapping (F, LPT) in one launch: blockIdx.z picks the bank.  Used by the
+// multirate plan for its low-rate banks, each of which is only a few microseconds of work.
+constexpr int kMaxMulti = 8;
+struct MultiFilterArgs {
+    FilterArgs bank[kMaxMulti];
+    int gx[kMaxMulti], gy[kMaxMulti];
+};
+
+template <int F, int LPT>
+__global__ void __launch_bounds__(kMaxWarps * 32) spiir_filter_multi_kernel(const __grid_constant__ MultiFilterArgs m)
+{
+    const int k = blockIdx.z;
+    if ((int)blockIdx.x >= m.gx[k] || (int)blockIdx.y >= m.gy[k]) return;
+    filter_body<F, LPT, false>(m.bank[k], blockIdx.x, blockIdx.y, m.gx[k], m.gy[k]);
 }
 
 // ---------------------------------------------------------------------------------------------

@@ -86,6 +86,8 @@ struct spiir_resamp {
 namespace spiir {
 spiir_status plan_geometry(const spiir_plan* p, int n, FilterGeometry* g);
 spiir_status filter_launch(spiir_plan* p, const float* x, int n, spiir_c64* z, int accumulate, cudaStream_t st);
+spiir_status filter_launch_group(spiir_plan* const* ps, const float* const* xs, const int* ns, spiir_c64* const* zs, int count,
+                                 cudaStream_t st);
 spiir_status down_chain_launch(spiir_resamp* const* downs, int nstages, const float* x, int n, float* const* xh,
                                int n_streams, cudaStream_t st);
 spiir_status up_chain_launch(spiir_resamp* const* ups, int nstages, const spiir_c64* z_low, int n_low,

@@ -3,6 +3,8 @@
 //   acc_{H-1} = z_{H-1};  acc_{h-1} = z_{h-1} + up2(acc_h);   result acc_0 (base rate).
 // Every stage keeps its own streaming history, so consecutive calls continue one stream.
 #include <algorithm>
+#include <stdio.h>
+#include <time.h>
 #include <new>
 #include <vector>
 
@@ -135,13 +137,48 @@ spiir_status spiir_mr_filter(spiir_mr_plan_t* p, const float* x, int n, spiir_c6
         }
     } else if (rc != SPIIR_OK) return rc;
     SPIIR_CUDA(cudaEventRecord(p->ev_chain, st));
-    for (int h = 1; h < p->H; ++h) {                       // row a9: per-rate banks, side by side
+#ifdef MR_TRACE
+    static double tr[4]; static int ntr = 0;
+    auto now = []() { timespec ts; clock_gettime(CLOCK_MONOTONIC, &ts); return ts.tv_sec * 1e6 + ts.tv_nsec * 1e-3; };
+    cudaDeviceSynchronize(); double t1 = now();
+#endif
+    // row a9: per-rate banks, side by side.  Unchunked banks that share a lane mapping go out as ONE launch
+    // (the low rates are a few microseconds of work each); everything else gets its own side stream.
+    std::vector<char> done(p->H, 0), rec(p->H, 0);
+    rec[0] = 1;
+    for (int h = 1; h < p->H; ++h) {
+        if (done[h]) continue;
+        FilterGeometry gh;
+        if ((rc = plan_geometry(p->banks[h], n >> h, &gh)) != SPIIR_OK) return rc;
+        std::vector<int> grp(1, h);
+        if (gh.NC == 1)
+            for (int j = h + 1; j < p->H && (int)grp.size() < 8; ++j) {
+                FilterGeometry gj;
+                if (done[j] || plan_geometry(p->banks[j], n >> j, &gj) != SPIIR_OK) continue;
+                if (gj.NC == 1 && gj.F == gh.F && gj.LPT == gh.LPT) grp.push_back(j);
+            }
         SPIIR_CUDA(cudaStreamWaitEvent(p->side[h], p->ev_chain, 0));
-        rc = filter_launch(p->banks[h], p->d_x[h], n >> h, p->d_z[h], 0, p->side[h]);
-        if (rc != SPIIR_OK) return rc;
+        rc = SPIIR_EUNSUPPORTED;
+        if (grp.size() >= 2) {
+            spiir_plan* ps[8]; const float* xs[8]; int ns[8]; spiir_c64* zs[8];
+            for (size_t k = 0; k < grp.size(); ++k) { ps[k] = p->banks[grp[k]]; xs[k] = p->d_x[grp[k]]; ns[k] = n >> grp[k]; zs[k] = p->d_z[grp[k]]; }
+            rc = filter_launch_group(ps, xs, ns, zs, (int)grp.size(), p->side[h]);
+            if (rc == SPIIR_OK) for (int j : grp) done[j] = 1;
+            else if (rc != SPIIR_EUNSUPPORTED) return rc;
+        }
+        if (rc == SPIIR_EUNSUPPORTED) {
+            rc = filter_launch(p->banks[h], p->d_x[h], n >> h, p->d_z[h], 0, p->side[h]);
+            if (rc != SPIIR_OK) return rc;
+            done[h] = 1;
+        }
         SPIIR_CUDA(cudaEventRecord(p->ev_bank[h], p->side[h]));
+        rec[h] = 1;
     }
-    for (int h = 0; h < p->H; ++h) SPIIR_CUDA(cudaStreamWaitEvent(st, p->ev_bank[h], 0));   // join
+    for (int h = 0; h < p->H; ++h)                                                         // join
+        if (rec[h]) SPIIR_CUDA(cudaStreamWaitEvent(st, p->ev_bank[h], 0));
+#ifdef MR_TRACE
+    cudaDeviceSynchronize(); double t2 = now();
+#endif
     // row a10: up + accumulate cascade, lowest rate first; one launch when the tap count has a fused kernel
     {
         const int nst = p->H - 1;
@@ -160,6 +197,11 @@ spiir_status spiir_mr_filter(spiir_mr_plan_t* p, const float* x, int n, spiir_c6
             }
         } else if (rc != SPIIR_OK) return rc;
     }
+#ifdef MR_TRACE
+    cudaDeviceSynchronize(); double t3 = now();
+    tr[1] += t2 - t1; tr[2] += t3 - t2; ++ntr;
+    if (ntr % 20 == 0) { fprintf(stderr, "MR_TRACE banks1..H-1 %.1f us  up chain %.1f us (avg of 20)\n", tr[1] / 20, tr[2] / 20); tr[1] = tr[2] = 0; }
+#endif
     return SPIIR_OK;
 }
 
@@ -179,10 +221,20 @@ int spiir_mr_launches(const spiir_mr_plan_t* p, int n)
     int total = p->H > 1 ? 2 : 0;                         // fused down chain + fused up cascade
     if (p->H > 1 && p->downs[0]->N != 192) total += p->H - 2;
     if (p->H > 1 && p->ups[0]->N != 192 && p->ups[0]->N != 32) total += p->H - 2;
+    std::vector<FilterGeometry> g(p->H);
+    for (int h = 0; h < p->H; ++h)
+        if (plan_geometry(p->banks[h], std::max(1, n >> h), &g[h]) != SPIIR_OK) return 0;
+    std::vector<char> done(p->H, 0);
     for (int h = 0; h < p->H; ++h) {
-        FilterGeometry g;
-        if (plan_geometry(p->banks[h], std::max(1, n >> h), &g) != SPIIR_OK) return 0;
-        total += g.launches;
+        if (done[h]) continue;
+        total += g[h].launches;
+        done[h] = 1;
+        // the same grouping as spiir_mr_filter: unchunked banks h >= 1 with one warp per template and F <= 8
+        if (h >= 1 && g[h].NC == 1 && g[h].LPT == 32 && g[h].F <= 8) {
+            int members = 1;
+            for (int j = h + 1; j < p->H && members < 8; ++j)
+                if (!done[j] && g[j].NC == 1 && g[j].F == g[h].F && g[j].LPT == g[h].LPT) { done[j] = 1; ++members; }
+        }
     }
     return total;
 }
