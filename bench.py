@@ -319,6 +319,11 @@ def bench_ours(args):
                                    f"{sm_max_mhz:.0f} MHz (clocks.max.sm, MEASURED_PEAKS.json); 12 flop per update (PAPER.md:88)"}
         # FMA-pipe view: an update needs 8 FP32 lane-ops (4 packed FFMA2-class instructions); the pipe peak is
         # SMs x 128 lane-ops per clock, so pipe utilisation = updates/s * 8 / (SMs * 128 * clock)
+        try:
+            roofline["peak_measured_ffma_loop"] = sp.spiir_probe_fp32_peak()      # TFLOP/s of a register-only FFMA loop
+            roofline["frac_of_measured"] = achieved / roofline["peak_measured_ffma_loop"]
+        except Exception:
+            pass
         roofline["fma_pipe_frac"] = (upd / (ms_per_step * 1e-3)) * 8.0 / (props.multi_processor_count * FP32_LANES_PER_SM * sm_max_mhz * 1e6)
         snr_bytes = S * T * n * 8
         cpu = None

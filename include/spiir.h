@@ -170,6 +170,12 @@ spiir_status spiir_host_layout(const spiir_c64* a1, const spiir_c64* b0, const i
 spiir_status spiir_host_geometry(int n_templates, int n_filters, int n_streams, int max_delay, int n,
                                  int time_chunks, int n_sm, int smem_optin, int info[8]);
 
+/* Measurement aid (not part of the hot path): times a register-only FFMA loop on the current device and
+ * returns the FP32 rate it reached in TFLOP/s (2 flop per FMA).  Synchronises the device.  bench.py reports
+ * the ALU roofline against the nominal peak (SMs x 128 lanes x 2 x clock) and quotes this number beside it
+ * ("achieved FP32 peak"). */
+spiir_status spiir_probe_fp32_peak(double* tflops_out);
+
 const char*  spiir_last_error(void);
 /* "spiir-b200 <version> sm_100a" */
 const char*  spiir_version(void);

@@ -28,7 +28,7 @@ EXPORTS = (
     "spiir_plan_get_state", "spiir_plan_set_state", "spiir_kaiser_taps", "spiir_resamp_create",
     "spiir_resample_down", "spiir_resample_up", "spiir_resamp_reset", "spiir_resamp_destroy",
     "spiir_mr_plan_create", "spiir_mr_filter", "spiir_mr_plan_reset", "spiir_mr_plan_destroy",
-    "spiir_mr_launches", "spiir_host_layout", "spiir_host_geometry", "spiir_last_error", "spiir_version",
+    "spiir_mr_launches", "spiir_probe_fp32_peak", "spiir_host_layout", "spiir_host_geometry", "spiir_last_error", "spiir_version",
 )
 
 
@@ -81,6 +81,7 @@ def lib():
         L.spiir_mr_plan_destroy.argtypes = [vp]
         L.spiir_mr_plan_destroy.restype = None
         L.spiir_mr_launches.argtypes = [vp, ci]
+        L.spiir_probe_fp32_peak.argtypes = [ctypes.POINTER(cd)]
         L.spiir_host_layout.argtypes = [vp, vp, vp, ci, ci, ci, vp, vp, vp, ctypes.POINTER(ci * 4),
                                         ctypes.POINTER(cd)]
         L.spiir_host_geometry.argtypes = [ci, ci, ci, ci, ci, ci, ci, ci, ctypes.POINTER(ci * 8)]
@@ -113,6 +114,13 @@ def _bank_arrays(a1, b0, delays):
 
 def version() -> str:
     return lib().spiir_version().decode()
+
+
+def spiir_probe_fp32_peak() -> float:
+    """TFLOP/s reached by a register-only FFMA loop on the current device (measurement aid)."""
+    v = ctypes.c_double(0.0)
+    _check(lib().spiir_probe_fp32_peak(ctypes.byref(v)), "spiir_probe_fp32_peak")
+    return float(v.value)
 
 
 def spiir_kaiser_taps(n_taps: int = 192, kaiser_beta: float = 5.0, cutoff: float = 0.25) -> np.ndarray:

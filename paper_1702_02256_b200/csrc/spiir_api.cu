@@ -482,6 +482,56 @@ spiir_status spiir_resample_up(spiir_resamp_t* r, const spiir_c64* in, int n_in,
     return SPIIR_OK;
 }
 
+
+// ---------------------------------------------------------------------------------------------
+// FP32 FMA peak probe (measurement aid for bench.py's ALU roofline; not on the hot path): every thread
+// runs 16 independent FFMA chains; returns 2 flop x FFMAs / time of the best of 5 launches.
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(1024) spiir_fp32_probe_kernel(float* out, int iters, float c0, float c1)
+{
+    float a[16];
+#pragma unroll
+    for (int i = 0; i < 16; ++i) a[i] = threadIdx.x * 1e-3f + i;
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int r = 0; r < 4; ++r)
+#pragma unroll
+            for (int i = 0; i < 16; ++i) a[i] = fmaf(a[i], c0, c1);
+    }
+    float s = 0.f;
+#pragma unroll
+    for (int i = 0; i < 16; ++i) s += a[i];
+    out[blockIdx.x * blockDim.x + threadIdx.x] = s;
+}
+
+spiir_status spiir_probe_fp32_peak(double* tflops_out)
+{
+    if (!tflops_out) { set_error("spiir_probe_fp32_peak: NULL"); return SPIIR_EINVAL; }
+    DeviceInfo dev;
+    spiir_status rc = device_info(&dev);
+    if (rc != SPIIR_OK) return rc;
+    const int blocks = dev.n_sm * 2, threads = 1024, iters = 4096;
+    float* d = nullptr;
+    SPIIR_CUDA(cudaMalloc(&d, (size_t)blocks * threads * sizeof(float)));
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0); cudaEventCreate(&e1);
+    float best = 1e30f;
+    for (int r = 0; r < 6; ++r) {
+        cudaEventRecord(e0);
+        spiir_fp32_probe_kernel<<<blocks, threads>>>(d, iters, 0.999f, 1e-3f);
+        cudaEventRecord(e1);
+        cudaError_t e = cudaEventSynchronize(e1);
+        if (e != cudaSuccess) { cudaFree(d); return cuda_fail(e, "spiir_probe_fp32_peak"); }
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, e0, e1);
+        if (r > 0 && ms < best) best = ms;
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(d);
+    const double fma = (double)blocks * threads * (double)iters * 64.0;
+    *tflops_out = 2.0 * fma / (best * 1e-3) / 1e12;
+    return SPIIR_OK;
+}
+
 }  // extern "C"
 
 namespace spiir {

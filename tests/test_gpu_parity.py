@@ -400,6 +400,41 @@ def test_kaiser_taps_match_oracle_design(sp, oracle_mod):
 
 
 # ------------------------------------------------------------------------------------------------
+# the five configs at their FULL sizes and FULL block counts, oracle on sampled templates
+# (templates are independent units; the tolerance is over the whole run, reading F10)
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("cfg,kw,nblk,idx", [
+    (1, {}, 16, [0, 1, 7, 500, 1023]),
+    (2, {"n_filters": 1}, 64, [0, 17, 2048, 4095]),
+    (2, {"n_filters": 4}, 64, [0, 17, 2048, 4095]),
+    (2, {"n_filters": 32}, 64, [0, 17, 2048, 4095]),
+    (3, {}, 32, [0, 511, 1023]),
+    (4, {}, 64, [0, 8191, 16383]),
+])
+def test_full_size_full_length_streams_sampled(sp, oracle_mod, cfg, kw, nblk, idx):
+    import torch
+    w = _inputs().config(cfg, **kw)
+    idx = np.array(idx)
+    if len(w.banks) == 1:
+        b = w.banks[0]
+        plan = sp.Plan(b.a1, b.b0, b.delays, b.rate_hz, n_streams=w.n_streams, max_block=w.block)
+        orc = oracle_mod.FilterOracle(b.a1[idx], b.b0[idx], b.delays[idx], w.n_streams)
+    else:
+        banks = [(b.a1, b.b0, b.delays) for b in w.banks]
+        plan = sp.MultiratePlan(banks, [b.rate_hz for b in w.banks], n_streams=w.n_streams, max_block=w.block)
+        orc = oracle_mod.MultirateOracle([(a[idx], b0[idx], d[idx]) for a, b0, d in banks], w.n_streams)
+    assert nblk == w.n_blocks
+    out = torch.empty((w.n_streams, w.n_templates, w.block), dtype=torch.complex64, device="cuda")
+    zs, refs = [], []
+    for i in range(nblk):
+        x = w.strain(i)
+        plan.filter(torch.from_numpy(x).cuda(), out)
+        zs.append(out[:, idx].cpu().numpy())
+        refs.append(orc.filter(x))
+    assert_parity(np.concatenate(zs, -1), np.concatenate(refs, -1), f"{w.name} full length")
+
+
+# ------------------------------------------------------------------------------------------------
 # CUDA graphs: the ping-pong phase of every carried history lives on the device, so one captured
 # call can be replayed for every block of a stream
 # ------------------------------------------------------------------------------------------------
