@@ -214,7 +214,8 @@ def bench_ours(args):
     # a captured call can be replayed for each block of the stream); eager launches if capture fails.
     def capture(xbuf, obuf):
         g = torch.cuda.CUDAGraph()
-        with torch.cuda.graph(g):
+        # thread_local: CUDA calls of other threads (NCCL watchdog, clock sampler) must not invalidate the capture
+        with torch.cuda.graph(g, capture_error_mode="thread_local"):
             plan.filter(xbuf, obuf)
         return g
 
