@@ -83,6 +83,21 @@ def test_lane_mapping(sp, L, F, LPT):
     assert F * LPT >= L
 
 
+def test_chunking_follows_the_cost_model(sp):
+    # configs[2]: 4096 templates x 8 filters, 256-sample blocks -> two more launches never pay
+    for L in (1, 2, 4, 8, 16, 32):
+        g = sp.spiir_host_geometry(4096, L, 1, 255, 256)
+        assert g["time_chunks"] == 1 and g["launches"] == 1, L
+    # the two highest rates of configs[3]: 1024 templates x 8 / 16 filters, 4096 / 2048 samples -> chunked
+    assert sp.spiir_host_geometry(1024, 8, 1, 4095, 4096)["time_chunks"] > 1
+    assert sp.spiir_host_geometry(1024, 16, 1, 2047, 2048)["time_chunks"] > 1
+    # ... but not its lower rates (one warp per template already gives 1024 warps)
+    assert sp.spiir_host_geometry(1024, 32, 1, 1023, 1024)["time_chunks"] == 1
+    # a long block of a small bank is chunked, a short one is not
+    assert sp.spiir_host_geometry(16, 128, 1, 2047, 4096)["time_chunks"] > 1
+    assert sp.spiir_host_geometry(16, 128, 1, 2047, 128)["time_chunks"] == 1
+
+
 def test_lane_mapping_many_templates(sp):
     # 32..128 filters and at least 16 x 148 templates: two templates per warp, 16 lanes each
     g = sp.spiir_host_geometry(4096, 64, 1, 100, 1024)
