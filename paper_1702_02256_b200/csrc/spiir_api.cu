@@ -442,6 +442,21 @@ spiir_status spiir_resample_up(spiir_resamp_t* r, const spiir_c64* in, int n_in,
         set_error("spiir_resample_up: out must be 16-byte and in 8-byte aligned");
         return SPIIR_EINVAL;
     }
+    if (r->N == 32) {
+        // short filter: HBM-bound streaming kernel, no shared memory
+        UpArgs u;
+        u.in = reinterpret_cast<const float2*>(in); u.out = reinterpret_cast<float2*>(out);
+        u.hbuf[0] = reinterpret_cast<float2*>(r->d_hist[0]); u.hbuf[1] = reinterpret_cast<float2*>(r->d_hist[1]);
+        u.phase = r->d_phase;
+        u.rows = r->rows; u.n_in = n_in; u.accumulate = accumulate;
+        u.seg = u.nseg = u.upr = u.rpc = 0;
+        const long long units = (long long)r->rows * ((n_in + kUpSR - 1) / kUpSR);
+        UpTaps<16> t;
+        for (int q = 0; q < 16; ++q) { t.t0[q] = r->taps[2 * q]; t.t1[q] = r->taps[2 * q + 1]; }
+        spiir_up2_stream_kernel<16><<<(unsigned)((units + 255) / 256), 256, 0, static_cast<cudaStream_t>(cuda_stream)>>>(u, t);
+        SPIIR_CUDA(cudaGetLastError());
+        return SPIIR_OK;
+    }
     if (r->N == 192 || r->N == 32) {
         // register-blocked kernel, taps in the kernel parameters (constant bank)
         UpArgs u;

@@ -286,6 +286,82 @@ __global__ void __launch_bounds__(128, 8) spiir_up2_fir_kernel(const UpArgs a, c
 }
 
 // ---------------------------------------------------------------------------------------------
+// Streaming up-by-2 (+ accumulate) for SHORT filters (32 taps: 32 FMA per 20 bytes, HBM-bound).
+//
+// No shared memory and no CTA-wide phases: a thread owns R = 4 consecutive input positions, reads the
+// R + HALF inputs it needs as 16-byte loads straight from global memory (neighbouring threads overlap,
+// the L1 serves the re-reads), fetches the 8 outputs it accumulates into, and writes 8 outputs.  With
+// ~100 bytes of DRAM traffic in flight per thread and 1024+ threads per SM the memory system stays busy
+// without any staging.  Taps are kernel parameters (constant bank).
+// ---------------------------------------------------------------------------------------------
+constexpr int kUpSR = 4;
+
+template <int HALF>
+__global__ void __launch_bounds__(256) spiir_up2_stream_kernel(const UpArgs a, const __grid_constant__ UpTaps<HALF> taps)
+{
+    constexpr int R = kUpSR, H = HALF - 1;
+    static_assert(HALF % 2 == 0, "the aligned fast path reads HALF + R inputs as pairs");
+    const int ph = phase_read(a.phase);
+    const float2* hcur = a.hbuf[ph];
+    float2* hnext = a.hbuf[ph ^ 1];
+    const int upr = (a.n_in + R - 1) / R;                                // units per row
+    const long long id = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const int row = (int)(id / upr), unit = (int)(id - (long long)row * upr);
+    if (row < a.rows) {
+        const int m0 = unit * R;
+        const float2* in = a.in + (size_t)row * a.n_in;
+        float2 v[R + HALF];                                             // v[i] = input m0 - HALF + i  (v[0] unused by the FIR)
+        if (m0 >= HALF && m0 + R <= a.n_in && (a.n_in & 1) == 0) {
+            const float4* p = reinterpret_cast<const float4*>(in + m0 - HALF);
+#pragma unroll
+            for (int i = 0; i < (R + HALF) / 2; ++i) {
+                const float4 q = p[i];
+                v[2 * i] = make_float2(q.x, q.y);
+                v[2 * i + 1] = make_float2(q.z, q.w);
+            }
+        } else {
+            const float2* hist = hcur + (size_t)row * H;
+#pragma unroll
+            for (int i = 0; i < R + HALF; ++i) {
+                const int g = m0 - HALF + i;
+                float2 x = make_float2(0.f, 0.f);
+                if (g >= 0) { if (g < a.n_in) x = in[g]; }
+                else if (H + g >= 0) x = hist[H + g];
+                v[i] = x;
+            }
+        }
+        float4* o = reinterpret_cast<float4*>(a.out + (size_t)row * 2 * a.n_in) + m0;
+        float4 old[R];
+#pragma unroll
+        for (int r = 0; r < R; ++r)
+            old[r] = (a.accumulate && m0 + r < a.n_in) ? o[r] : make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            float2 acc0 = make_float2(0.f, 0.f), acc1 = make_float2(0.f, 0.f);
+#pragma unroll
+            for (int q = 0; q < HALF; ++q) {
+                const float2 x = v[HALF + r - q];                       // input m0 + r - q
+                acc0.x = fmaf(taps.t0[q], x.x, acc0.x);
+                acc0.y = fmaf(taps.t0[q], x.y, acc0.y);
+                acc1.x = fmaf(taps.t1[q], x.x, acc1.x);
+                acc1.y = fmaf(taps.t1[q], x.y, acc1.y);
+            }
+            if (m0 + r < a.n_in)
+                o[r] = make_float4(fmaf(2.f, acc0.x, old[r].x), fmaf(2.f, acc0.y, old[r].y),
+                                   fmaf(2.f, acc1.x, old[r].z), fmaf(2.f, acc1.y, old[r].w));
+        }
+        // carried history: the first H units of a row copy one sample each (last H inputs of hist ++ in)
+        if (H > 0) {
+            for (int i = unit; i < H; i += upr) {
+                const int g = a.n_in - H + i;
+                hnext[(size_t)row * H + i] = (g >= 0) ? in[g] : hcur[(size_t)row * H + a.n_in + i];
+            }
+        }
+    }
+    if (last_cta_arrives(a.phase, gridDim.x)) a.phase[0] = ph ^ 1;
+}
+
+// ---------------------------------------------------------------------------------------------
 // Register-blocked down-by-2 for a compile-time tap count N (real rows).
 //
 // A thread owns R = 10 consecutive outputs; they depend on N + 2R - 2 consecutive inputs, fetched
