@@ -4,6 +4,7 @@
 #include <string.h>
 
 #include <algorithm>
+#include <mutex>
 #include <new>
 #include <vector>
 
@@ -33,18 +34,23 @@ spiir_status device_info(DeviceInfo* out)
 // limit only when a launch needs more than any earlier one did (per device the limit only grows).
 static cudaError_t ensure_smem(const void* func, int bytes)
 {
-    static const void* funcs[128];
-    static int limits[128];
+    static std::mutex mu;
+    static const void* funcs[256];
+    static int devs[256], limits[256];
     static int nfuncs = 0;
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);                 // the attribute is per device
+    if (e != cudaSuccess) return e;
+    std::lock_guard<std::mutex> lock(mu);
     for (int i = 0; i < nfuncs; ++i)
-        if (funcs[i] == func) {
+        if (funcs[i] == func && devs[i] == dev) {
             if (limits[i] >= bytes) return cudaSuccess;
-            cudaError_t e = cudaFuncSetAttribute(func, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+            e = cudaFuncSetAttribute(func, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
             if (e == cudaSuccess) limits[i] = bytes;
             return e;
         }
-    cudaError_t e = cudaFuncSetAttribute(func, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
-    if (e == cudaSuccess && nfuncs < 128) { funcs[nfuncs] = func; limits[nfuncs] = bytes; ++nfuncs; }
+    e = cudaFuncSetAttribute(func, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    if (e == cudaSuccess && nfuncs < 256) { funcs[nfuncs] = func; devs[nfuncs] = dev; limits[nfuncs] = bytes; ++nfuncs; }
     return e;
 }
 
