@@ -233,10 +233,10 @@ __global__ void __launch_bounds__(128, 8) spiir_up2_fir_kernel(const UpArgs a, c
             for (int r = 0; r < R; ++r) {
                 const int q = r - (R - 1) + jj;                         // tap pair index of position r
                 if (q >= 0 && q < HALF) {
-                    acc0[r].x = fmaf(taps.t0[q], v.x, acc0[r].x);
-                    acc0[r].y = fmaf(taps.t0[q], v.y, acc0[r].y);
-                    acc1[r].x = fmaf(taps.t1[q], v.x, acc1[r].x);
-                    acc1[r].y = fmaf(taps.t1[q], v.y, acc1[r].y);
+                    // packed (re, im) FMA with the tap as a broadcast uniform-register operand: half the issue
+                    // slots of four scalar FFMAs, so the loads and index arithmetic issue in their shadow
+                    acc0[r] = __ffma2_rn(make_float2(taps.t0[q], taps.t0[q]), v, acc0[r]);
+                    acc1[r] = __ffma2_rn(make_float2(taps.t1[q], taps.t1[q]), v, acc1[r]);
                 }
             }
         }
@@ -341,10 +341,8 @@ __global__ void __launch_bounds__(256) spiir_up2_stream_kernel(const UpArgs a, c
 #pragma unroll
             for (int q = 0; q < HALF; ++q) {
                 const float2 x = v[HALF + r - q];                       // input m0 + r - q
-                acc0.x = fmaf(taps.t0[q], x.x, acc0.x);
-                acc0.y = fmaf(taps.t0[q], x.y, acc0.y);
-                acc1.x = fmaf(taps.t1[q], x.x, acc1.x);
-                acc1.y = fmaf(taps.t1[q], x.y, acc1.y);
+                acc0 = __ffma2_rn(make_float2(taps.t0[q], taps.t0[q]), x, acc0);
+                acc1 = __ffma2_rn(make_float2(taps.t1[q], taps.t1[q]), x, acc1);
             }
             if (m0 + r < a.n_in)
                 o[r] = make_float4(fmaf(2.f, acc0.x, old[r].x), fmaf(2.f, acc0.y, old[r].y),
@@ -588,10 +586,8 @@ __global__ void __launch_bounds__(128, 7) spiir_up_chain_kernel(const UpChainArg
                 for (int r = 0; r < R; ++r) {
                     const int q = r - (R - 1) + jj;
                     if (q >= 0 && q < HALF) {
-                        acc0[r].x = fmaf(taps.t0[q], v.x, acc0[r].x);
-                        acc0[r].y = fmaf(taps.t0[q], v.y, acc0[r].y);
-                        acc1[r].x = fmaf(taps.t1[q], v.x, acc1[r].x);
-                        acc1[r].y = fmaf(taps.t1[q], v.y, acc1[r].y);
+                        acc0[r] = __ffma2_rn(make_float2(taps.t0[q], taps.t0[q]), v, acc0[r]);
+                        acc1[r] = __ffma2_rn(make_float2(taps.t1[q], taps.t1[q]), v, acc1[r]);
                     }
                 }
             }
