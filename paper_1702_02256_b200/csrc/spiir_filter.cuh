@@ -277,7 +277,9 @@ __device__ __forceinline__ void filter_body(const FilterArgs& a, const int bx, c
         }
     }
     const int ntiles = (tc1 - tc0 + a.NT - 1) / a.NT;
-    if (ntiles == 1) stage_window(win, bar, parity, a, hist_s, x_s, tc0);
+    // single-tile case: the window is staged once, AFTER the first group's coefficient / state loads have been
+    // issued (below), so that their DRAM round trip overlaps the TMA copy and the shifted copies
+    bool staged = ntiles != 1;
     const float4* win4 = reinterpret_cast<const float4*>(win);
 
     constexpr int TPG = 32 / LPT;                                       // templates per group
@@ -304,6 +306,7 @@ __device__ __forceinline__ void filter_body(const FilterArgs& a, const int bx, c
             Y[f] = y0;
         }
         float2* zt = active ? a.z + ((size_t)s * a.T + t) * (size_t)a.n : nullptr;
+        if (!staged) { stage_window(win, bar, parity, a, hist_s, x_s, tc0); staged = true; }
 
         for (int tile = 0; tile < ntiles; ++tile) {
             const int t0 = tc0 + tile * a.NT;
