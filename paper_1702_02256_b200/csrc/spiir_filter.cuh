@@ -57,8 +57,9 @@ __device__ __forceinline__ bool last_cta_arrives(int* w, int total_ctas)
 {
     __syncthreads();
     bool last = false;
+    // No fence: nothing written by this launch is read before the launch has ended (the flipped phase and the
+    // history it points to are consumed by the NEXT launch); a fence would wait for the CTA's SNR stores to drain.
     if (threadIdx.x == 0) {
-        __threadfence();
         last = atomicAdd(w + 1, 1) == total_ctas - 1;
         if (last) w[1] = 0;
     }
