@@ -33,6 +33,11 @@
  *     stream at a time; plans are not thread-safe.
  *   - Errors: argument errors return SPIIR_EINVAL and enqueue nothing; CUDA failures return
  *     SPIIR_ECUDA / SPIIR_ENOMEM.  spiir_last_error() gives a thread-local message.
+ *   - A compute call enqueues the SAME kernels with the SAME arguments for every block of a stream
+ *     (which half of each ping-pong history is current is a word in device memory, flipped by the
+ *     kernels themselves), so one call captured into a CUDA graph can be replayed for every block
+ *     as long as x / snr_out / n stay the same.  The multirate call forks onto plan-owned side
+ *     streams with events and joins before it returns control of `cuda_stream` (capturable).
  *   - There is no CPU fallback: without a CUDA device every create call fails with SPIIR_ECUDA.
  *   - Arithmetic is IEEE float32 with FMA contraction; the sum over filters is taken in a fixed,
  *     plan-determined order (deterministic, reading F8).
