@@ -422,7 +422,7 @@ def bench_resample(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=48)
+    ap.add_argument("--steps", type=int, default=200)
     ap.add_argument("--warmup", type=int, default=16)
     ap.add_argument("--config", type=int, default=1, help="BASELINE.json configs index (default 1: the metric's config)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
