@@ -622,4 +622,24 @@ spiir_status up_chain_launch(spiir_resamp* const* ups, int nstages, const spiir_
     return SPIIR_OK;
 }
 
+
+// Whether the fused chains can serve a block of n base-rate samples (same conditions as the launchers).
+bool down_chain_fits(spiir_resamp* const* downs, int nstages, int n)
+{
+    if (nstages < 1 || nstages > kMaxStages || downs[0]->N != 192) return false;
+    size_t words = 0;
+    for (int k = 0; k <= nstages; ++k) words += down_chain_buf_len(192, n >> k);
+    return words * sizeof(float) <= (size_t)downs[0]->dev.smem_optin;
+}
+
+bool up_chain_fits(spiir_resamp* const* ups, int nstages, int n_low)
+{
+    if (nstages < 1 || nstages > kMaxStages) return false;
+    const int N = ups[0]->N;
+    if (N != 192 && N != 32) return false;
+    const size_t cap = (size_t)up_chain_buf_len(N / 2, n_low << (nstages - 1)) +
+                       (size_t)up_chain_buf_len(N / 2, nstages >= 2 ? n_low << (nstages - 2) : 1);
+    return cap * sizeof(float2) <= (size_t)ups[0]->dev.smem_optin;
+}
+
 }  // namespace spiir

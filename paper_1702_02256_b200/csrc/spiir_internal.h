@@ -90,6 +90,8 @@ spiir_status filter_launch_group(spiir_plan* const* ps, const float* const* xs, 
                                  cudaStream_t st);
 spiir_status down_chain_launch(spiir_resamp* const* downs, int nstages, const float* x, int n, float* const* xh,
                                int n_streams, cudaStream_t st);
+bool down_chain_fits(spiir_resamp* const* downs, int nstages, int n);
+bool up_chain_fits(spiir_resamp* const* ups, int nstages, int n_low);
 spiir_status up_chain_launch(spiir_resamp* const* ups, int nstages, const spiir_c64* z_low, int n_low,
                              const spiir_c64* const* z_add, spiir_c64* out, int rows, cudaStream_t st);
 }  // namespace spiir

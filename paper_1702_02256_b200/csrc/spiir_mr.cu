@@ -218,9 +218,14 @@ spiir_status spiir_mr_plan_reset(spiir_mr_plan_t* p, void* cuda_stream)
 int spiir_mr_launches(const spiir_mr_plan_t* p, int n)
 {
     if (!p || n < 1) return 0;
-    int total = p->H > 1 ? 2 : 0;                         // fused down chain + fused up cascade
-    if (p->H > 1 && p->downs[0]->N != 192) total += p->H - 2;
-    if (p->H > 1 && p->ups[0]->N != 192 && p->ups[0]->N != 32) total += p->H - 2;
+    int total = 0;
+    if (p->H > 1) {
+        // fused down chain / fused up cascade when they apply (tap count, shared memory), else one launch per stage
+        total += down_chain_fits(p->downs.data(), p->H - 1, n) ? 1 : p->H - 1;
+        std::vector<spiir_resamp*> ups(p->H - 1);
+        for (int k = 0; k < p->H - 1; ++k) ups[k] = p->ups[p->H - 2 - k];
+        total += up_chain_fits(ups.data(), p->H - 1, n >> (p->H - 1)) ? 1 : p->H - 1;
+    }
     std::vector<FilterGeometry> g(p->H);
     for (int h = 0; h < p->H; ++h)
         if (plan_geometry(p->banks[h], std::max(1, n >> h), &g[h]) != SPIIR_OK) return 0;

@@ -392,6 +392,27 @@ def test_multirate_two_streams(sp, oracle_mod):
     np.testing.assert_array_equal(z1[0], z[1])
 
 
+def test_multirate_long_block_falls_back_to_per_stage_launches(sp, oracle_mod):
+    """A block too long for the fused chains' shared-memory buffers: one launch per stage instead
+    (and the banks tile their windows in time)."""
+    inp = _inputs()
+    rates = [4096, 2048, 1024]
+    banks = []
+    for h, (R, L) in enumerate(zip(rates, (6, 20, 40))):
+        b = inp.make_bank((9, 9, h), 3, L, R, 0.9, 0.9999, 300)
+        banks.append((b.a1, b.b0, b.delays))
+    n = 65536
+    plan = sp.MultiratePlan(banks, rates, max_block=n)
+    # 65536 samples: 2 + 2 per-stage resampling launches (the fused chains would need > 227 KB) + >= 1 per bank
+    assert plan.launches(n) >= 4 + 3
+    orc = oracle_mod.MultirateOracle(banks)
+    rng = np.random.default_rng(3)
+    xs = [rng.standard_normal((1, m)).astype(np.float32) for m in (n, 4096)]
+    z = stream_gpu_plan(plan, xs)
+    ref = stream_oracle(orc, xs)
+    assert_parity(z, ref, "multirate long block")
+
+
 def test_kaiser_taps_match_oracle_design(sp, oracle_mod):
     """The library generates its own taps (no shared table); they agree with the oracle's to 1 ulp."""
     h = sp.spiir_kaiser_taps(192, 5.0, 0.25)
