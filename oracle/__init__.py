@@ -174,13 +174,18 @@ class MultirateOracle:
     across calls.  banks: list over rates (highest first) of (a1, b0, delays), each [T][L_h].
     """
 
-    def __init__(self, banks, n_streams: int = 1, n_taps: int = 192, beta: float = 5.0, cutoff: float = 0.25):
+    def __init__(self, banks, n_streams: int = 1, n_taps: int = 192, beta: float = 5.0, cutoff: float = 0.25,
+                 n_taps_down=None, beta_down=None, cutoff_down=None, n_taps_up=None, beta_up=None, cutoff_up=None):
+        """n_taps / beta / cutoff: one filter for both directions (BASELINE.json configs[3]); the *_down /
+        *_up arguments override it per direction (~100 dB / 384 taps down, ~60 dB / 32 taps up)."""
         self.H, self.S = len(banks), int(n_streams)
         self.T = np.asarray(banks[0][0]).shape[0]
-        taps32 = kaiser_taps(n_taps, beta, cutoff)[1]
+        pick = lambda v, dflt: dflt if v is None else v
+        taps_d = kaiser_taps(pick(n_taps_down, n_taps), pick(beta_down, beta), pick(cutoff_down, cutoff))[1]
+        taps_u = kaiser_taps(pick(n_taps_up, n_taps), pick(beta_up, beta), pick(cutoff_up, cutoff))[1]
         self.filters = [FilterOracle(a1, b0, d, n_streams) for (a1, b0, d) in banks]
-        self.downs = [ResampOracle("down", self.S, taps32) for _ in range(self.H - 1)]
-        self.ups = [ResampOracle("up", self.S * self.T, taps32) for _ in range(self.H - 1)]
+        self.downs = [ResampOracle("down", self.S, taps_d) for _ in range(self.H - 1)]
+        self.ups = [ResampOracle("up", self.S * self.T, taps_u) for _ in range(self.H - 1)]
 
     def filter(self, x) -> np.ndarray:
         x = np.ascontiguousarray(x, dtype=np.float64)

@@ -164,6 +164,25 @@ def test_block_streaming_equals_one_run(cuts):
     assert np.array_equal(o.filter(x), ref)
 
 
+@pytest.mark.parametrize("cuts", [[23, 5, 41, 130, 1], [17] * 9, [3, 90, 2, 58]])
+def test_two_streams_streamed_equal_each_stream_alone(cuts):
+    """Per-stream history carry (hist + s*D) and per-stream state: S = 2 streamed over ragged blocks,
+    some shorter than d_max = 60, must equal (bitwise) the S = 1 oracle run on each stream alone in
+    ONE call, and the S = 2 one-call run.  Mixing up the two histories or states fails this."""
+    a1, b0, d = small_bank(15, dmax=60)
+    n = sum(cuts)
+    x = np.random.default_rng(16).standard_normal((2, n))
+    o = FilterOracle(a1, b0, d, n_streams=2)
+    pos, outs = 0, []
+    for c in cuts:
+        outs.append(o.filter(x[:, pos:pos + c])); pos += c
+    got = np.concatenate(outs, axis=2)
+    assert np.array_equal(got, FilterOracle(a1, b0, d, n_streams=2).filter(x))
+    for s in range(2):
+        assert np.array_equal(got[s], FilterOracle(a1, b0, d).filter(x[s])[0])
+    assert not np.array_equal(got[0], got[1])
+
+
 # ---- O4 taps ---------------------------------------------------------------------------------
 
 def test_taps_match_numpy_kaiser_times_sinc():
@@ -211,6 +230,25 @@ def test_up2_equals_zero_stuff_convolve():
         stuffed = np.zeros(600, complex); stuffed[0::2] = v[r]
         ref = 2 * np.convolve(stuffed, h32.astype(np.float64))[:600]
         assert np.allclose(out[r], ref, rtol=1e-12, atol=1e-14)
+
+
+@pytest.mark.parametrize("n_taps,beta", [(32, 5.0), (384, 10.0), (64, 7.0)])
+def test_resamplers_other_tap_counts_equal_numpy_convolve(n_taps, beta):
+    """384 taps down / 32 taps up are the paper's own filter lengths; the resamplers
+    must stay the plain convolution for any even N (history N-1 / N/2-1, streamed in ragged blocks)."""
+    _, h32 = kaiser_taps(n_taps, beta, 0.25)
+    h = h32.astype(np.float64)
+    rng = np.random.default_rng(n_taps)
+    u = rng.standard_normal((2, 900))
+    v = rng.standard_normal((2, 450)) + 1j * rng.standard_normal((2, 450))
+    od = ResampOracle("down", 2, n_taps=n_taps, beta=beta)
+    ou = ResampOracle("up", 2, n_taps=n_taps, beta=beta)
+    got_d = np.concatenate([od.down(u[:, a:b]) for a, b in ((0, 2), (2, 300), (300, 900))], axis=1)
+    got_u = np.concatenate([ou.up(v[:, a:b]) for a, b in ((0, 1), (1, 7), (7, 450))], axis=1)
+    for r in range(2):
+        assert np.allclose(got_d[r], np.convolve(u[r], h)[0:900:2], rtol=1e-12, atol=1e-14)
+        stuffed = np.zeros(900, complex); stuffed[0::2] = v[r]
+        assert np.allclose(got_u[r], 2 * np.convolve(stuffed, h)[:900], rtol=1e-12, atol=1e-14)
 
 
 def test_up2_accumulate_adds():
@@ -294,6 +332,38 @@ def test_multirate_streams_in_blocks():
     o = MultirateOracle(banks)
     got = np.concatenate([o.filter(x[i:i + 256]) for i in range(0, 1024, 256)], axis=2)
     assert np.array_equal(got, ref)
+
+
+def test_multirate_two_streams_streamed_equal_each_stream_alone():
+    """MultirateOracle(n_streams=2): the rows = S*T reshape of the up cascade and the per-stream FIR /
+    bank histories, streamed over ragged blocks (multiples of 2^(H-1) = 4, some shorter than the
+    delays and FIR histories), equal the S = 1 oracle on each stream alone in one call (bitwise)."""
+    banks = mr_banks(36, 3, [3, 2, 4], [40, 25, 12])
+    n = 1024
+    x = np.random.default_rng(37).standard_normal((2, n))
+    o = MultirateOracle(banks, n_streams=2)
+    cuts, pos, outs = [4, 60, 256, 8, 696], 0, []
+    for c in cuts:
+        outs.append(o.filter(x[:, pos:pos + c])); pos += c
+    got = np.concatenate(outs, axis=2)
+    assert got.shape == (2, 3, n)
+    for s in range(2):
+        assert np.array_equal(got[s], MultirateOracle(banks).filter(x[s])[0])
+    assert not np.array_equal(got[0], got[1])
+
+
+def test_multirate_separate_down_up_taps_cascade_equals_direct():
+    """different filters per direction (384-tap down, 32-tap up).  Same linearity pin
+    as above with the two tap sets passed separately."""
+    T, n = 2, 512
+    banks = mr_banks(38, T, [3, 4], [20, 10])
+    x = np.random.default_rng(39).standard_normal(n)
+    kw = dict(n_taps_down=384, beta_down=10.0, n_taps_up=32, beta_up=5.0)
+    got = MultirateOracle(banks, **kw).filter(x)
+    x1 = ResampOracle("down", 1, n_taps=384, beta=10.0).down(x[None, :])
+    z0 = FilterOracle(*banks[0]).filter(x)[0]
+    z1 = ResampOracle("up", T, n_taps=32, beta=5.0).up(FilterOracle(*banks[1]).filter(x1)[0])
+    assert np.allclose(got[0], z0 + z1, rtol=1e-12, atol=1e-14)
 
 
 def test_oracle_reports_threads():
