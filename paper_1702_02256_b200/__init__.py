@@ -24,11 +24,16 @@ SPIIR_OK, SPIIR_EINVAL, SPIIR_ENOMEM, SPIIR_ECUDA, SPIIR_EUNSUPPORTED, SPIIR_EST
 SPIIR_DOWN2, SPIIR_UP2 = 0, 1
 
 EXPORTS = (
-    "spiir_plan_create", "spiir_filter", "spiir_plan_reset", "spiir_plan_destroy", "spiir_plan_launch_info",
-    "spiir_plan_get_state", "spiir_plan_set_state", "spiir_kaiser_taps", "spiir_resamp_create",
-    "spiir_resample_down", "spiir_resample_up", "spiir_resamp_reset", "spiir_resamp_destroy",
-    "spiir_mr_plan_create", "spiir_mr_filter", "spiir_mr_plan_reset", "spiir_mr_plan_destroy",
-    "spiir_mr_launches", "spiir_probe_fp32_peak", "spiir_host_layout", "spiir_host_geometry", "spiir_last_error", "spiir_version",
+    "spiir_plan_workspace_bytes", "spiir_plan_create", "spiir_plan_workspace_bytes_ragged", "spiir_plan_create_ragged",
+    "spiir_filter", "spiir_plan_reset", "spiir_plan_destroy", "spiir_plan_launch_info",
+    "spiir_plan_history_len", "spiir_plan_get_state", "spiir_plan_set_state", "spiir_kaiser_taps",
+    "spiir_resamp_workspace_bytes", "spiir_resamp_create", "spiir_resample_down", "spiir_resample_up", "spiir_resamp_reset",
+    "spiir_resamp_destroy", "spiir_resamp_history_len", "spiir_resamp_get_state", "spiir_resamp_set_state",
+    "spiir_mr_workspace_bytes", "spiir_mr_plan_create", "spiir_mr_filter", "spiir_mr_plan_reset", "spiir_mr_plan_destroy",
+    "spiir_mr_launches", "spiir_mr_plan_state_bytes", "spiir_mr_plan_get_state", "spiir_mr_plan_set_state",
+    "spiir_assign_rates", "spiir_host_layout", "spiir_host_geometry", "spiir_host_lane_mapping",
+    "spiir_pd_plan_create", "spiir_pd_filter", "spiir_pd_plan_reset", "spiir_pd_plan_destroy",
+    "spiir_probe_fp32_peak", "spiir_probe_ffma2_operands", "spiir_last_error", "spiir_version",
 )
 
 
@@ -41,12 +46,18 @@ class SpiirError(RuntimeError):
 
 class _PlanOpts(ctypes.Structure):
     _fields_ = [("n_streams", ctypes.c_int), ("max_block", ctypes.c_int), ("time_chunks", ctypes.c_int),
-                ("flags", ctypes.c_int)]
+                ("flags", ctypes.c_int), ("workspace", ctypes.c_void_p), ("workspace_bytes", ctypes.c_size_t)]
+
+
+class _ResampOpts(ctypes.Structure):
+    _fields_ = [("max_block", ctypes.c_int), ("workspace", ctypes.c_void_p), ("workspace_bytes", ctypes.c_size_t)]
 
 
 class _MrOpts(ctypes.Structure):
-    _fields_ = [("n_streams", ctypes.c_int), ("max_block", ctypes.c_int), ("n_taps", ctypes.c_int),
-                ("kaiser_beta", ctypes.c_double), ("cutoff", ctypes.c_double)]
+    _fields_ = [("n_streams", ctypes.c_int), ("max_block", ctypes.c_int),
+                ("n_taps_down", ctypes.c_int), ("kaiser_beta_down", ctypes.c_double), ("cutoff_down", ctypes.c_double),
+                ("n_taps_up", ctypes.c_int), ("kaiser_beta_up", ctypes.c_double), ("cutoff_up", ctypes.c_double),
+                ("workspace", ctypes.c_void_p), ("workspace_bytes", ctypes.c_size_t)]
 
 
 def lib():
@@ -57,23 +68,36 @@ def lib():
             raise RuntimeError(f"{LIB_PATH} is missing: build it with `python -m paper_1702_02256_b200.build` "
                                "(there is no CPU or PyTorch fallback for the SPIIR hot path)")
         L = ctypes.CDLL(LIB_PATH)
-        vp, ci, cd = ctypes.c_void_p, ctypes.c_int, ctypes.c_double
+        vp, ci, cd, sz = ctypes.c_void_p, ctypes.c_int, ctypes.c_double, ctypes.c_size_t
         pvp = ctypes.POINTER(vp)
+        L.spiir_plan_workspace_bytes.argtypes = [ci, ci, ci, ci, ci, ci]
+        L.spiir_plan_workspace_bytes.restype = sz
+        L.spiir_plan_workspace_bytes_ragged.argtypes = [vp, ci, ci, ci, ci, ci]
+        L.spiir_plan_workspace_bytes_ragged.restype = sz
         L.spiir_plan_create.argtypes = [pvp, vp, vp, vp, ci, ci, ci, ctypes.POINTER(_PlanOpts)]
+        L.spiir_plan_create_ragged.argtypes = [pvp, vp, vp, vp, vp, ci, ci, ctypes.POINTER(_PlanOpts)]
         L.spiir_filter.argtypes = [vp, vp, ci, vp, vp]
         L.spiir_plan_reset.argtypes = [vp, vp]
         L.spiir_plan_destroy.argtypes = [vp]
         L.spiir_plan_destroy.restype = None
         L.spiir_plan_launch_info.argtypes = [vp, ci, ctypes.POINTER(ci * 8)]
-        L.spiir_plan_get_state.argtypes = [vp, vp, vp]
-        L.spiir_plan_set_state.argtypes = [vp, vp, vp]
+        L.spiir_plan_history_len.argtypes = [vp]
+        L.spiir_plan_get_state.argtypes = [vp, vp, vp, vp]
+        L.spiir_plan_set_state.argtypes = [vp, vp, vp, vp]
         L.spiir_kaiser_taps.argtypes = [ci, cd, cd, vp]
-        L.spiir_resamp_create.argtypes = [pvp, ci, ci, cd, cd, ci, ci]
+        L.spiir_resamp_workspace_bytes.argtypes = [ci, ci, ci]
+        L.spiir_resamp_workspace_bytes.restype = sz
+        L.spiir_resamp_create.argtypes = [pvp, ci, ci, cd, cd, ci, ctypes.POINTER(_ResampOpts)]
         L.spiir_resample_down.argtypes = [vp, vp, ci, vp, vp]
         L.spiir_resample_up.argtypes = [vp, vp, ci, vp, ci, vp]
         L.spiir_resamp_reset.argtypes = [vp, vp]
         L.spiir_resamp_destroy.argtypes = [vp]
         L.spiir_resamp_destroy.restype = None
+        L.spiir_resamp_history_len.argtypes = [vp]
+        L.spiir_resamp_get_state.argtypes = [vp, vp, vp]
+        L.spiir_resamp_set_state.argtypes = [vp, vp, vp]
+        L.spiir_mr_workspace_bytes.argtypes = [ci, ctypes.POINTER(ci), ctypes.POINTER(ci), ci, ctypes.POINTER(_MrOpts)]
+        L.spiir_mr_workspace_bytes.restype = sz
         L.spiir_mr_plan_create.argtypes = [pvp, ci, ctypes.POINTER(ci), pvp, pvp, pvp, ctypes.POINTER(ci), ci,
                                            ctypes.POINTER(_MrOpts)]
         L.spiir_mr_filter.argtypes = [vp, vp, ci, vp, vp]
@@ -81,10 +105,22 @@ def lib():
         L.spiir_mr_plan_destroy.argtypes = [vp]
         L.spiir_mr_plan_destroy.restype = None
         L.spiir_mr_launches.argtypes = [vp, ci]
+        L.spiir_mr_plan_state_bytes.argtypes = [vp]
+        L.spiir_mr_plan_state_bytes.restype = sz
+        L.spiir_mr_plan_get_state.argtypes = [vp, vp, vp]
+        L.spiir_mr_plan_set_state.argtypes = [vp, vp, vp]
+        L.spiir_assign_rates.argtypes = [vp, ci, ci, ctypes.POINTER(ci), ci, cd, vp]
+        L.spiir_pd_plan_create.argtypes = [pvp, vp, vp, vp, ci, ci, ci]
+        L.spiir_pd_filter.argtypes = [vp, vp, ci, vp, vp]
+        L.spiir_pd_plan_reset.argtypes = [vp, vp]
+        L.spiir_pd_plan_destroy.argtypes = [vp]
+        L.spiir_pd_plan_destroy.restype = None
         L.spiir_probe_fp32_peak.argtypes = [ctypes.POINTER(cd)]
+        L.spiir_probe_ffma2_operands.argtypes = [ctypes.POINTER(cd * 4)]
         L.spiir_host_layout.argtypes = [vp, vp, vp, ci, ci, ci, vp, vp, vp, ctypes.POINTER(ci * 4),
                                         ctypes.POINTER(cd)]
         L.spiir_host_geometry.argtypes = [ci, ci, ci, ci, ci, ci, ci, ci, ctypes.POINTER(ci * 8)]
+        L.spiir_host_lane_mapping.argtypes = [ci, ci, ctypes.POINTER(ci * 3)]
         L.spiir_last_error.restype = ctypes.c_char_p
         L.spiir_version.restype = ctypes.c_char_p
         _lib = L
@@ -123,10 +159,27 @@ def spiir_probe_fp32_peak() -> float:
     return float(v.value)
 
 
+def spiir_probe_ffma2_operands() -> dict:
+    """Cycles per packed FFMA2 warp-instruction when it reads 3 / 4 / 5 / 6 distinct register words (measurement aid)."""
+    v = (ctypes.c_double * 4)()
+    _check(lib().spiir_probe_ffma2_operands(ctypes.byref(v)), "spiir_probe_ffma2_operands")
+    return {"words3": v[0], "words4": v[1], "words5": v[2], "words6": v[3]}
+
+
 def spiir_kaiser_taps(n_taps: int = 192, kaiser_beta: float = 5.0, cutoff: float = 0.25) -> np.ndarray:
     out = np.empty(n_taps, dtype=np.float32)
     _check(lib().spiir_kaiser_taps(n_taps, kaiser_beta, cutoff, out.ctypes.data), "spiir_kaiser_taps")
     return out
+
+
+def spiir_assign_rates(a1, base_rate_hz: int, rates_hz: Sequence[int], band_factor: float = 1.0) -> np.ndarray:
+    """Rate index of every filter from its a1 (reading R8).  Host only."""
+    a1 = np.ascontiguousarray(a1, dtype=np.complex64)
+    rates = (ctypes.c_int * len(rates_hz))(*[int(r) for r in rates_hz])
+    out = np.empty(a1.size, dtype=np.int32)
+    _check(lib().spiir_assign_rates(a1.ctypes.data, a1.size, int(base_rate_hz), rates, len(rates_hz), float(band_factor),
+                                    out.ctypes.data), "spiir_assign_rates")
+    return out.reshape(a1.shape)
 
 
 def spiir_host_layout(a1, b0, delays, avoid_conflicts: bool = True):
@@ -159,18 +212,69 @@ def spiir_host_geometry(n_templates, n_filters, n_streams, max_delay, n, time_ch
     return dict(zip(_INFO_KEYS, list(info)))
 
 
+def spiir_host_lane_mapping(n_filters: int, n_templates: int = 1) -> dict:
+    info = (ctypes.c_int * 3)()
+    _check(lib().spiir_host_lane_mapping(int(n_filters), int(n_templates), ctypes.byref(info)), "spiir_host_lane_mapping")
+    return {"F": info[0], "lanes_per_template": info[1], "warps_per_template": info[2]}
+
+
+def _workspace(nbytes: int, device=None):
+    """One torch tensor that the plan borrows for its lifetime: every device byte of a plan comes from PyTorch."""
+    import torch
+    if nbytes <= 0:
+        raise SpiirError(SPIIR_EUNSUPPORTED, "workspace size query")
+    return torch.empty(int(nbytes), dtype=torch.uint8, device=device or "cuda")
+
+
+def _need(t, dtype, numel, what):
+    if not (t.is_cuda and t.dtype == dtype and t.is_contiguous() and t.numel() == numel):
+        raise ValueError(f"{what} must be a contiguous CUDA {dtype} tensor of {numel} elements")
+
+
 class Plan:
-    """Single-rate SPIIR bank with carried state (spiir_plan_create / spiir_filter)."""
+    """Single-rate SPIIR bank with carried state (spiir_plan_create / spiir_filter).
+
+    Uniform bank: ``Plan(a1, b0, delays)`` with [T][L] arrays.  Ragged bank (spiir_plan_create_ragged):
+    ``Plan.ragged(a1_flat, b0_flat, delays_flat, filter_offsets)``.  The device workspace is a torch tensor."""
 
     def __init__(self, a1, b0, delays, rate_hz: int = 4096, n_streams: int = 1, max_block: int = 4096,
-                 time_chunks: int = 0, flags: int = 0):
-        a1, b0, d = _bank_arrays(a1, b0, delays)
-        self.T, self.L = a1.shape
+                 time_chunks: int = 0, flags: int = 0, _offsets=None):
+        import torch
         self.S, self.max_block, self.rate_hz = int(n_streams), int(max_block), int(rate_hz)
-        opts = _PlanOpts(self.S, self.max_block, int(time_chunks), int(flags))
+        self.device = torch.device("cuda", torch.cuda.current_device()) if torch.cuda.is_available() else None
         self._h = ctypes.c_void_p()
-        _check(lib().spiir_plan_create(ctypes.byref(self._h), a1.ctypes.data, b0.ctypes.data, d.ctypes.data,
-                                       self.T, self.L, self.rate_hz, ctypes.byref(opts)), "spiir_plan_create")
+        if _offsets is None:
+            a1, b0, d = _bank_arrays(a1, b0, delays)
+            self.T, self.L = a1.shape
+            self.n_filters_total = self.T * self.L
+            need = lib().spiir_plan_workspace_bytes(self.T, self.L, int(d.max(initial=0)), self.S, self.max_block, int(time_chunks))
+            self._ws = _workspace(need) if need else None
+            opts = _PlanOpts(self.S, self.max_block, int(time_chunks), int(flags),
+                             self._ws.data_ptr() if self._ws is not None else None, need)
+            _check(lib().spiir_plan_create(ctypes.byref(self._h), a1.ctypes.data, b0.ctypes.data, d.ctypes.data,
+                                           self.T, self.L, self.rate_hz, ctypes.byref(opts)), "spiir_plan_create")
+        else:
+            a1 = np.ascontiguousarray(a1, dtype=np.complex64).ravel()
+            b0 = np.ascontiguousarray(b0, dtype=np.complex64).ravel()
+            d = np.ascontiguousarray(delays, dtype=np.int32).ravel()
+            off = np.ascontiguousarray(_offsets, dtype=np.int32)
+            if off.ndim != 1 or off.size < 2 or a1.size != off[-1] or b0.size != a1.size or d.size != a1.size:
+                raise ValueError("ragged bank: flat arrays must have filter_offsets[-1] entries")
+            self.T, self.L = off.size - 1, None
+            self.n_filters_total = int(off[-1])
+            need = lib().spiir_plan_workspace_bytes_ragged(off.ctypes.data, self.T, int(d.max(initial=0)), self.S, self.max_block,
+                                                           int(time_chunks))
+            self._ws = _workspace(need) if need else None
+            opts = _PlanOpts(self.S, self.max_block, int(time_chunks), int(flags),
+                             self._ws.data_ptr() if self._ws is not None else None, need)
+            _check(lib().spiir_plan_create_ragged(ctypes.byref(self._h), a1.ctypes.data, b0.ctypes.data, d.ctypes.data,
+                                                  off.ctypes.data, self.T, self.rate_hz, ctypes.byref(opts)),
+                   "spiir_plan_create_ragged")
+        self.history_len = int(lib().spiir_plan_history_len(self._h))
+
+    @classmethod
+    def ragged(cls, a1_flat, b0_flat, delays_flat, filter_offsets, **kw):
+        return cls(a1_flat, b0_flat, delays_flat, _offsets=filter_offsets, **kw)
 
     def filter(self, x, out=None, stream=None):
         """x: CUDA float32 [n] or [S][n]; returns (or fills) CUDA complex64 [S][T][n]."""
@@ -184,9 +288,8 @@ class Plan:
         n = int(x.shape[1])
         if out is None:
             out = torch.empty((self.S, self.T, n), dtype=torch.complex64, device=x.device)
-        elif not (out.is_cuda and out.dtype == torch.complex64 and out.is_contiguous()
-                  and out.numel() == self.S * self.T * n):
-            raise ValueError("out must be a contiguous CUDA complex64 tensor of S*T*n elements")
+        else:
+            _need(out, torch.complex64, self.S * self.T * n, "out")
         _check(lib().spiir_filter(self._h, x.data_ptr(), n, out.data_ptr(), _stream_ptr(stream)), "spiir_filter")
         return out
 
@@ -199,22 +302,28 @@ class Plan:
         return dict(zip(_INFO_KEYS, list(info)))
 
     def get_state(self, stream=None):
+        """(y, hist): filter state complex64 [S][T][L] (ragged: [S][total filters]) and the last history_len inputs."""
         import torch
-        y = torch.empty((self.S, self.T, self.L), dtype=torch.complex64, device="cuda")
-        _check(lib().spiir_plan_get_state(self._h, y.data_ptr(), _stream_ptr(stream)), "spiir_plan_get_state")
-        return y
+        shape = (self.S, self.T, self.L) if self.L is not None else (self.S, self.n_filters_total)
+        y = torch.empty(shape, dtype=torch.complex64, device=self.device)
+        hist = torch.empty((self.S, self.history_len), dtype=torch.float32, device=self.device)
+        _check(lib().spiir_plan_get_state(self._h, y.data_ptr(), hist.data_ptr() if self.history_len else None,
+                                          _stream_ptr(stream)), "spiir_plan_get_state")
+        return y, hist
 
-    def set_state(self, y, stream=None) -> None:
+    def set_state(self, y, hist, stream=None) -> None:
         import torch
-        if not (y.is_cuda and y.dtype == torch.complex64 and y.is_contiguous()
-                and tuple(y.shape) == (self.S, self.T, self.L)):
-            raise ValueError("y must be a contiguous CUDA complex64 [S][T][L] tensor")
-        _check(lib().spiir_plan_set_state(self._h, y.data_ptr(), _stream_ptr(stream)), "spiir_plan_set_state")
+        _need(y, torch.complex64, self.S * self.n_filters_total, "y")
+        if self.history_len:
+            _need(hist, torch.float32, self.S * self.history_len, "hist")
+        _check(lib().spiir_plan_set_state(self._h, y.data_ptr(), hist.data_ptr() if self.history_len else None,
+                                          _stream_ptr(stream)), "spiir_plan_set_state")
 
     def close(self) -> None:
         if getattr(self, "_h", None) and _lib is not None:
             _lib.spiir_plan_destroy(self._h)
             self._h = None
+        self._ws = None
 
     def __del__(self):
         try:
@@ -229,9 +338,14 @@ class Resampler:
     def __init__(self, direction: str, n_rows: int, max_block: int, n_taps: int = 192, kaiser_beta: float = 5.0,
                  cutoff: float = 0.25):
         self.direction, self.rows, self.max_block = direction, int(n_rows), int(max_block)
+        code = {"down": SPIIR_DOWN2, "up": SPIIR_UP2}[direction]
+        need = lib().spiir_resamp_workspace_bytes(code, int(n_taps), self.rows)
+        self._ws = _workspace(need) if need else None
+        opts = _ResampOpts(self.max_block, self._ws.data_ptr() if self._ws is not None else None, need)
         self._h = ctypes.c_void_p()
-        _check(lib().spiir_resamp_create(ctypes.byref(self._h), {"down": SPIIR_DOWN2, "up": SPIIR_UP2}[direction],
-                                         n_taps, kaiser_beta, cutoff, self.rows, self.max_block), "spiir_resamp_create")
+        _check(lib().spiir_resamp_create(ctypes.byref(self._h), code, n_taps, kaiser_beta, cutoff, self.rows,
+                                         ctypes.byref(opts)), "spiir_resamp_create")
+        self.history_len = int(lib().spiir_resamp_history_len(self._h))
 
     def down(self, u, out=None, stream=None):
         import torch
@@ -239,9 +353,13 @@ class Resampler:
             raise ValueError("u must be a contiguous CUDA float32 tensor")
         if u.dim() == 1:
             u = u[None, :]
+        if self.direction != "down" or u.shape[0] != self.rows or u.shape[1] % 2:
+            raise ValueError("u must be [rows][even n_in] for a down stage")
         n_in = int(u.shape[1])
         if out is None:
             out = torch.empty((self.rows, n_in // 2), dtype=torch.float32, device=u.device)
+        else:
+            _need(out, torch.float32, self.rows * (n_in // 2), "out")
         _check(lib().spiir_resample_down(self._h, u.data_ptr(), n_in, out.data_ptr(), _stream_ptr(stream)),
                "spiir_resample_down")
         return out
@@ -252,14 +370,34 @@ class Resampler:
             raise ValueError("v must be a contiguous CUDA complex64 tensor")
         if v.dim() == 1:
             v = v[None, :]
+        if self.direction != "up" or v.shape[0] != self.rows:
+            raise ValueError("v must be [rows][n_in] for an up stage")
         n_in = int(v.shape[1])
         if out is None:
             if accumulate:
                 raise ValueError("accumulate needs an output tensor")
             out = torch.empty((self.rows, 2 * n_in), dtype=torch.complex64, device=v.device)
+        else:
+            _need(out, torch.complex64, self.rows * 2 * n_in, "out")
         _check(lib().spiir_resample_up(self._h, v.data_ptr(), n_in, out.data_ptr(), int(bool(accumulate)),
                                        _stream_ptr(stream)), "spiir_resample_up")
         return out
+
+    def get_state(self, stream=None):
+        import torch
+        dt = torch.float32 if self.direction == "down" else torch.complex64
+        h = torch.empty((self.rows, self.history_len), dtype=dt, device="cuda")
+        _check(lib().spiir_resamp_get_state(self._h, h.data_ptr() if self.history_len else None, _stream_ptr(stream)),
+               "spiir_resamp_get_state")
+        return h
+
+    def set_state(self, hist, stream=None) -> None:
+        import torch
+        dt = torch.float32 if self.direction == "down" else torch.complex64
+        if self.history_len:
+            _need(hist, dt, self.rows * self.history_len, "hist")
+        _check(lib().spiir_resamp_set_state(self._h, hist.data_ptr() if self.history_len else None, _stream_ptr(stream)),
+               "spiir_resamp_set_state")
 
     def reset(self, stream=None) -> None:
         _check(lib().spiir_resamp_reset(self._h, _stream_ptr(stream)), "spiir_resamp_reset")
@@ -268,6 +406,7 @@ class Resampler:
         if getattr(self, "_h", None) and _lib is not None:
             _lib.spiir_resamp_destroy(self._h)
             self._h = None
+        self._ws = None
 
     def __del__(self):
         try:
@@ -278,10 +417,12 @@ class Resampler:
 
 class MultiratePlan:
     """Multirate SPIIR (spiir_mr_plan_create / spiir_mr_filter).  banks: highest rate first, each
-    (a1, b0, delays) of shape [T][L_h]; rates_hz descending, each half of the previous."""
+    (a1, b0, delays) of shape [T][L_h]; rates_hz descending, each half of the previous.  n_taps / kaiser_beta /
+    cutoff set both directions; the *_down / *_up arguments override one."""
 
     def __init__(self, banks: Sequence, rates_hz: Sequence[int], n_streams: int = 1, max_block: Optional[int] = None,
-                 n_taps: int = 192, kaiser_beta: float = 5.0, cutoff: float = 0.25):
+                 n_taps: int = 192, kaiser_beta: float = 5.0, cutoff: float = 0.25, n_taps_down=None, kaiser_beta_down=None,
+                 cutoff_down=None, n_taps_up=None, kaiser_beta_up=None, cutoff_up=None):
         arrs = [_bank_arrays(*b) for b in banks]
         H = len(arrs)
         self.H, self.T, self.S = H, arrs[0][0].shape[0], int(n_streams)
@@ -291,8 +432,15 @@ class MultiratePlan:
         b0p = (vp * H)(*[a[1].ctypes.data for a in arrs])
         dp = (vp * H)(*[a[2].ctypes.data for a in arrs])
         nf = (ctypes.c_int * H)(*[a[0].shape[1] for a in arrs])
+        dmax = (ctypes.c_int * H)(*[int(a[2].max(initial=0)) for a in arrs])
         rates = (ctypes.c_int * H)(*[int(r) for r in rates_hz])
-        opts = _MrOpts(self.S, self.max_block, n_taps, kaiser_beta, cutoff)
+        pick = lambda v, d: d if v is None else v
+        opts = _MrOpts(self.S, self.max_block, int(pick(n_taps_down, n_taps)), float(pick(kaiser_beta_down, kaiser_beta)),
+                       float(pick(cutoff_down, cutoff)), int(pick(n_taps_up, n_taps)), float(pick(kaiser_beta_up, kaiser_beta)),
+                       float(pick(cutoff_up, cutoff)), None, 0)
+        need = lib().spiir_mr_workspace_bytes(H, nf, dmax, self.T, ctypes.byref(opts))
+        self._ws = _workspace(need) if need else None
+        opts.workspace, opts.workspace_bytes = (self._ws.data_ptr() if self._ws is not None else None), need
         self._h = ctypes.c_void_p()
         _check(lib().spiir_mr_plan_create(ctypes.byref(self._h), H, rates, a1p, b0p, dp, nf, self.T,
                                           ctypes.byref(opts)), "spiir_mr_plan_create")
@@ -303,14 +451,30 @@ class MultiratePlan:
             raise ValueError("x must be a contiguous CUDA float32 tensor")
         if x.dim() == 1:
             x = x[None, :]
+        if x.shape[0] != self.S:
+            raise ValueError("x must be [S][n]")
         n = int(x.shape[1])
         if out is None:
             out = torch.empty((self.S, self.T, n), dtype=torch.complex64, device=x.device)
+        else:
+            _need(out, torch.complex64, self.S * self.T * n, "out")
         _check(lib().spiir_mr_filter(self._h, x.data_ptr(), n, out.data_ptr(), _stream_ptr(stream)), "spiir_mr_filter")
         return out
 
     def launches(self, n: int) -> int:
         return int(lib().spiir_mr_launches(self._h, int(n)))
+
+    def get_state(self, stream=None):
+        """The whole resume state (every bank's y and history, every FIR history) as one uint8 device blob."""
+        import torch
+        blob = torch.empty(int(lib().spiir_mr_plan_state_bytes(self._h)), dtype=torch.uint8, device="cuda")
+        _check(lib().spiir_mr_plan_get_state(self._h, blob.data_ptr(), _stream_ptr(stream)), "spiir_mr_plan_get_state")
+        return blob
+
+    def set_state(self, blob, stream=None) -> None:
+        import torch
+        _need(blob, torch.uint8, int(lib().spiir_mr_plan_state_bytes(self._h)), "blob")
+        _check(lib().spiir_mr_plan_set_state(self._h, blob.data_ptr(), _stream_ptr(stream)), "spiir_mr_plan_set_state")
 
     def reset(self, stream=None) -> None:
         _check(lib().spiir_mr_plan_reset(self._h, _stream_ptr(stream)), "spiir_mr_plan_reset")
@@ -318,6 +482,46 @@ class MultiratePlan:
     def close(self) -> None:
         if getattr(self, "_h", None) and _lib is not None:
             _lib.spiir_mr_plan_destroy(self._h)
+            self._h = None
+        self._ws = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+class PaperDesignPlan:
+    """COMPARISON ONLY: the paper's own Maxwell kernel design on this GPU (spiir_pd_plan_create / spiir_pd_filter)."""
+
+    def __init__(self, a1, b0, delays, max_block: int = 4096):
+        a1, b0, d = _bank_arrays(a1, b0, delays)
+        self.T, self.L = a1.shape
+        self.max_block = int(max_block)
+        self._h = ctypes.c_void_p()
+        _check(lib().spiir_pd_plan_create(ctypes.byref(self._h), a1.ctypes.data, b0.ctypes.data, d.ctypes.data, self.T, self.L,
+                                          self.max_block), "spiir_pd_plan_create")
+
+    def filter(self, x, out=None, stream=None):
+        import torch
+        if not (x.is_cuda and x.dtype == torch.float32 and x.is_contiguous()):
+            raise ValueError("x must be a contiguous CUDA float32 tensor")
+        x = x.reshape(-1)
+        n = int(x.numel())
+        if out is None:
+            out = torch.empty((1, self.T, n), dtype=torch.complex64, device=x.device)
+        else:
+            _need(out, torch.complex64, self.T * n, "out")
+        _check(lib().spiir_pd_filter(self._h, x.data_ptr(), n, out.data_ptr(), _stream_ptr(stream)), "spiir_pd_filter")
+        return out
+
+    def reset(self, stream=None) -> None:
+        _check(lib().spiir_pd_plan_reset(self._h, _stream_ptr(stream)), "spiir_pd_plan_reset")
+
+    def close(self) -> None:
+        if getattr(self, "_h", None) and _lib is not None:
+            _lib.spiir_pd_plan_destroy(self._h)
             self._h = None
 
     def __del__(self):

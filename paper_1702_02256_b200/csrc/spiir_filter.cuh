@@ -11,14 +11,21 @@
 //     (re, im), x and the coefficients enter as broadcast operands -- 4 packed instructions per
 //     filter-sample update instead of 8 scalar ones.
 //   * Eq. 8: per lane the F filters are summed in registers; 16 time steps are batched and summed
-//     across the LPT lanes with a transposed butterfly (xor-shuffles), which leaves every lane
-//     with a distinct slice of the 16 complex outputs -> coalesced stores, fixed summation order.
+//     across the lanes of the template.  One warp per template (LPT = 32): a transposed reduction
+//     through a padded, conflict-free shared-memory tile (8 STS.128 + 8 LDS.128 per lane instead
+//     of 31 SHFL + 62 FSEL: the kernel is bound by register-file read bandwidth).
+//     Fewer lanes per template: a transposed xor-butterfly.  Either way every lane ends with a
+//     distinct slice of the 16 complex outputs -> coalesced stores, fixed summation order.
+//   * templates of more than 512 filters span NP adjacent warps of one CTA; their per-batch partial
+//     sums meet in shared memory behind a named barrier (the 513-filter example).
 //   * time-parallel mode (row a7): a block is cut into chunks; pass 1 runs every chunk from zero
 //     state (chunk 0 from the carried state), a carry kernel propagates s_{c+1} = a1^C s_c + e_c,
 //     pass 2 reruns every chunk from its true initial state and writes z.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
+
+#include "spiir_common.cuh"
 
 namespace spiir {
 
@@ -28,7 +35,8 @@ constexpr int kMaxWarps = 8;      // warps per CTA (launch bound 256 threads -> 
 struct FilterArgs {
     const float4* coef;      // [G][F][32]  (a1.re, a1.im, b0.re, b0.im), plan order
     const int*    dly;       // [G][F][32]  delay in samples
-    float2*       state;     // [S][G][F][32] carried y (in/out)
+    float2*       state;     // [S][sstride], this bank's [G][F][32] carried y (in/out) at the start of every row
+    size_t        sstride;   // elements between the state rows of two streams
     float2*       chunk_st;  // chunked modes: [S][NC][G][F][32]; pass 1 writes end states, carry
                              // turns them into initial states in place, pass 2 reads them
     float*        hbuf[2];   // [S][Dpad] input history, ping-pong: hbuf[phase] holds the Dpad samples before
@@ -46,24 +54,20 @@ struct FilterArgs {
     int mode;                // 0 plain, 1 chunk pass 1 (no z), 2 chunk pass 2
     int x_aligned;           // x rows are 16-byte aligned (x pointer and n*4) -> TMA path
     int accumulate;          // z += result instead of z = result
+    const int* tmap;         // ragged plans: output row of template t of this class (nullptr: row = t)
+    int T_rows;              // rows of z per stream (= T unless the bank is one class of a ragged plan)
+    int NP;                  // warps per template (LPT = 32 only; G = T * NP pieces)
+    int carry;               // this launch writes the next input history and flips the phase
 };
 
-// ---------------------------------------------------------------------------------------------
-// Ping-pong phase kept on the device.  A kernel reads w[0] when it starts; the CTA that finishes last
-// (arrival counter w[1]) flips it, so no CTA can observe the flip of its own launch.
-// ---------------------------------------------------------------------------------------------
-__device__ __forceinline__ int phase_read(const int* w) { return *reinterpret_cast<const volatile int*>(w) & 1; }
-__device__ __forceinline__ bool last_cta_arrives(int* w, int total_ctas)
+// shared-memory scratch of one warp for the transposed reduction (LPT = 32), in float4 units:
+// [32 rows][9] (a row = the lane's 16 complex partial sums + one float4 of padding) and [2][32] second-stage words
+constexpr int kRedRows4 = 32 * 9;
+constexpr int kRedWarp4 = kRedRows4 + 64;
+
+__device__ __forceinline__ void named_bar_sync(int id, int nthreads)
 {
-    __syncthreads();
-    bool last = false;
-    // No fence: nothing written by this launch is read before the launch has ended (the flipped phase and the
-    // history it points to are consumed by the NEXT launch); a fence would wait for the CTA's SNR stores to drain.
-    if (threadIdx.x == 0) {
-        last = atomicAdd(w + 1, 1) == total_ctas - 1;
-        if (last) w[1] = 0;
-    }
-    return last;                                     // meaningful in thread 0 only
+    asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -167,34 +171,65 @@ __device__ __forceinline__ void bfly_stage(float2* Z, int lane)
     }
 }
 
+struct RedCtx {
+    float4* rows;            // this warp's [32][9] tile
+    float4* part2;           // this warp's [2][32] second-stage words
+    int part, NP, bar_id;    // piece index within the template, pieces per template, named barrier of the template
+};
+
+// LPT = 32.  Every lane writes its 16 complex partial sums as one padded row; lane j then sums float quad (j & 7)
+// over the eight rows 4i + (j >> 3); the four partial quads of a column meet in a second tile, from which lane j
+// sums float j.  With NP > 1 the second tiles of the NP warps of a template are summed by its first warp after a
+// named barrier (double-buffered by the batch parity, so one barrier per batch suffices).
+__device__ __forceinline__ void reduce_store_warp(float2 (&Z)[kBatch], int lane, float2* zrow, int nvalid, bool active, bool acc,
+                                                  const RedCtx& rc, int bpar)
+{
+    float4* myrow = rc.rows + lane * 9;
+#pragma unroll
+    for (int q = 0; q < 8; ++q) myrow[q] = make_float4(Z[2 * q].x, Z[2 * q].y, Z[2 * q + 1].x, Z[2 * q + 1].y);
+    __syncwarp();
+    const float4* col = rc.rows + (lane >> 3) * 9 + (lane & 7);
+    float2 a0 = make_float2(0.f, 0.f), a1 = make_float2(0.f, 0.f);
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+        const float4 v = col[i * 36];
+        a0 = __fadd2_rn(a0, make_float2(v.x, v.y));
+        a1 = __fadd2_rn(a1, make_float2(v.z, v.w));
+    }
+    rc.part2[bpar * 32 + lane] = make_float4(a0.x, a0.y, a1.x, a1.y);
+    if (rc.NP == 1) __syncwarp();
+    else named_bar_sync(rc.bar_id, 32 * rc.NP);
+    if (rc.part != 0) return;
+    float v = 0.f;
+    for (int p = 0; p < rc.NP; ++p) {
+        const float* f = reinterpret_cast<const float*>(rc.part2 + (size_t)p * kRedWarp4 + bpar * 32);
+        const float w = (f[lane] + f[32 + lane]) + (f[64 + lane] + f[96 + lane]);
+        v = p == 0 ? w : v + w;
+    }
+    if (active && (lane >> 1) < nvalid) {
+        float* o = reinterpret_cast<float*>(zrow) + lane;
+        if (acc) v += *o;
+        *o = v;
+    }
+}
+
 template <int LPT>
 __device__ __forceinline__ void reduce_store(float2 (&Z)[kBatch], int lane, float2* zrow, int nvalid, bool active, bool acc)
 {
+    static_assert(LPT < 32, "one warp per template reduces through shared memory (reduce_store_warp)");
     // zrow: this lane's template row at the batch start (complex index), valid when active
     if (LPT >= 2)  bfly_stage<16, LPT / 2>(Z, lane);
     if (LPT >= 4)  bfly_stage<8, LPT / 4>(Z, lane);
     if (LPT >= 8)  bfly_stage<4, LPT / 8>(Z, lane);
     if (LPT >= 16) bfly_stage<2, LPT / 16>(Z, lane);
-    if (LPT == 32) {
-        const bool up = (lane & 1) != 0;
-        float keep = up ? Z[0].y : Z[0].x;
-        float send = up ? Z[0].x : Z[0].y;
-        float v = keep + __shfl_xor_sync(0xffffffffu, send, 1);
-        if (active && (lane >> 1) < nvalid) {
-            float* p = reinterpret_cast<float*>(zrow) + lane;
-            if (acc) v += *p;
-            *p = v;
-        }
-    } else {
-        constexpr int NV = kBatch / LPT;                  // complex values left per lane
-        const int base = (lane & (LPT - 1)) * NV;
+    constexpr int NV = kBatch / LPT;                  // complex values left per lane
+    const int base = (lane & (LPT - 1)) * NV;
 #pragma unroll
-        for (int i = 0; i < NV; ++i) {
-            if (active && base + i < nvalid) {
-                float2 v = Z[i];
-                if (acc) { float2 o = zrow[base + i]; v.x += o.x; v.y += o.y; }
-                zrow[base + i] = v;
-            }
+    for (int i = 0; i < NV; ++i) {
+        if (active && base + i < nvalid) {
+            float2 v = Z[i];
+            if (acc) { float2 o = zrow[base + i]; v.x += o.x; v.y += o.y; }
+            zrow[base + i] = v;
         }
     }
 }
@@ -254,6 +289,7 @@ __device__ __forceinline__ void filter_body(const FilterArgs& a, const int bx, c
     extern __shared__ __align__(16) unsigned char smem_raw[];
     float* win = reinterpret_cast<float*>(smem_raw);                   // 4 copies x CS floats
     uint64_t* bar = reinterpret_cast<uint64_t*>(win + 4 * (size_t)a.CS);
+    float4* red = reinterpret_cast<float4*>(win + 4 * (size_t)a.CS + 4);    // LPT = 32: kRedWarp4 float4 per warp
 
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
     const int s = by / a.NC, c = by % a.NC;
@@ -269,7 +305,7 @@ __device__ __forceinline__ void filter_body(const FilterArgs& a, const int bx, c
     // carried history for the next block (reads only hist + x: no race with other CTAs).  Every CTA of the
     // stream copies a slice: one CTA doing all Dpad samples is a chain of ~Dpad/blockDim dependent global
     // round trips (11 us for 4096 samples) that the whole launch then waits for.
-    if (a.mode != 1) {
+    if (a.carry) {
         float* hn = a.hbuf[ph ^ 1] + (size_t)s * a.Dpad;
         const int cta = c * gdx + bx, nctas = a.NC * gdx;
         for (int i = cta * blockDim.x + threadIdx.x; i < a.Dpad; i += nctas * blockDim.x) {
@@ -284,11 +320,18 @@ __device__ __forceinline__ void filter_body(const FilterArgs& a, const int bx, c
     const float4* win4 = reinterpret_cast<const float4*>(win);
 
     constexpr int TPG = 32 / LPT;                                       // templates per group
+    const int NP = LPT == 32 ? a.NP : 1;                                // warps per template (nwarps % NP == 0)
+    RedCtx rc;
+    rc.NP = NP; rc.part = warp % NP; rc.bar_id = 1 + warp / NP;
+    rc.rows = red + (size_t)warp * kRedWarp4;
+    rc.part2 = rc.rows + kRedRows4;      // the pieces of a template are adjacent warps: piece p's words sit p * kRedWarp4 on
+    int bcount = 0;                                                     // batches done (parity = second-stage buffer)
     for (int g0 = bx * nwarps; g0 < a.G; g0 += gdx * nwarps) {
-        const int g = g0 + warp;
+        const int g = g0 + warp;                                        // piece: template g / NP, part g % NP
         const bool wactive = g < a.G;
-        const int t = g * TPG + lane / LPT;
-        const bool active = wactive && t < a.T;
+        const int tl = (g / NP) * TPG + lane / LPT;                     // template within this bank
+        const bool active = wactive && tl < a.T;
+        const int t = active ? (a.tmap ? a.tmap[tl] : tl) : 0;          // output row
         float4 cf[F]; float2 Y[F]; int off4[F];
         const size_t lbase = ((size_t)(wactive ? g : 0) * F) * 32 + lane;
 #pragma unroll
@@ -300,13 +343,13 @@ __device__ __forceinline__ void filter_body(const FilterArgs& a, const int bx, c
             float2 y0 = make_float2(0.f, 0.f);
             if (wactive) {
                 if (a.mode == 0 || (a.mode == 1 && c == 0))
-                    y0 = a.state[((size_t)s * a.G * F) * 32 + lbase + (size_t)f * 32];
+                    y0 = a.state[(size_t)s * a.sstride + lbase + (size_t)f * 32];
                 else if (a.mode == 2)
                     y0 = a.chunk_st[(((size_t)s * a.NC + c) * a.G * F) * 32 + lbase + (size_t)f * 32];
             }
             Y[f] = y0;
         }
-        float2* zt = active ? a.z + ((size_t)s * a.T + t) * (size_t)a.n : nullptr;
+        float2* zt = active ? a.z + ((size_t)s * a.T_rows + t) * (size_t)a.n : nullptr;
         if (!staged) { stage_window(win, bar, parity, a, hist_s, x_s, tc0); staged = true; }
 
         for (int tile = 0; tile < ntiles; ++tile) {
@@ -317,29 +360,44 @@ __device__ __forceinline__ void filter_body(const FilterArgs& a, const int bx, c
             float2 Z[kBatch];
             for (int b = 0; b < nfull; ++b) {
                 batch_steps<F, true, NOZ>(win4, off4, b * (kBatch / 4), cf, Y, Z, kBatch);
-                if (!NOZ) reduce_store<LPT>(Z, lane, zt + t0 + b * kBatch, kBatch, active, a.accumulate != 0);
+                if (!NOZ) {
+                    if (LPT == 32) {
+                        reduce_store_warp(Z, lane, zt + t0 + b * kBatch, kBatch, active, a.accumulate != 0, rc, bcount & 1);
+                        ++bcount;
+                    } else {
+                        reduce_store<(LPT < 32 ? LPT : 16)>(Z, lane, zt + t0 + b * kBatch, kBatch, active, a.accumulate != 0);
+                    }
+                }
             }
             const int rem = len - nfull * kBatch;
             if (rem > 0) {
                 batch_steps<F, false, NOZ>(win4, off4, nfull * (kBatch / 4), cf, Y, Z, rem);
-                if (!NOZ) reduce_store<LPT>(Z, lane, zt + t0 + nfull * kBatch, rem, active, a.accumulate != 0);
+                if (!NOZ) {
+                    if (LPT == 32) {
+                        reduce_store_warp(Z, lane, zt + t0 + nfull * kBatch, rem, active, a.accumulate != 0, rc, bcount & 1);
+                        ++bcount;
+                    } else {
+                        reduce_store<(LPT < 32 ? LPT : 16)>(Z, lane, zt + t0 + nfull * kBatch, rem, active, a.accumulate != 0);
+                    }
+                }
             }
         }
         if (wactive) {
 #pragma unroll
             for (int f = 0; f < F; ++f) {
                 if (a.mode == 0 || (a.mode == 2 && c == a.NC - 1))
-                    a.state[((size_t)s * a.G * F) * 32 + lbase + (size_t)f * 32] = Y[f];
+                    a.state[(size_t)s * a.sstride + lbase + (size_t)f * 32] = Y[f];
                 else if (a.mode == 1)
                     a.chunk_st[(((size_t)s * a.NC + c) * a.G * F) * 32 + lbase + (size_t)f * 32] = Y[f];
             }
         }
     }
-    if (a.mode != 1 && last_cta_arrives(a.phase, gdx * gdy)) a.phase[0] = ph ^ 1;
+    if (a.carry && last_cta_arrives(a.phase, gdx * gdy)) a.phase[0] = ph ^ 1;
 }
 
+// F <= 8 is held to 128 registers so that two 8-warp CTAs (4 warps per scheduler) share an SM when their windows fit.
 template <int F, int LPT, bool NOZ>
-__global__ void __launch_bounds__(kMaxWarps * 32) spiir_filter_kernel(const FilterArgs a)
+__global__ void __launch_bounds__(kMaxWarps * 32, (F <= 8 ? 2 : 1)) spiir_filter_kernel(const FilterArgs a)
 {
     filter_body<F, LPT, NOZ>(a, blockIdx.x, blockIdx.y, gridDim.x, gridDim.y);
 }
@@ -353,7 +411,7 @@ struct MultiFilterArgs {
 };
 
 template <int F, int LPT>
-__global__ void __launch_bounds__(kMaxWarps * 32) spiir_filter_multi_kernel(const __grid_constant__ MultiFilterArgs m)
+__global__ void __launch_bounds__(kMaxWarps * 32, 2) spiir_filter_multi_kernel(const __grid_constant__ MultiFilterArgs m)
 {
     const int k = blockIdx.z;
     if ((int)blockIdx.x >= m.gx[k] || (int)blockIdx.y >= m.gy[k]) return;
@@ -366,7 +424,7 @@ __global__ void __launch_bounds__(kMaxWarps * 32) spiir_filter_multi_kernel(cons
 //   after : chunk_st[c] = true INITIAL state of chunk c  (chunk_st[0] = carried state)
 // s_{c+1} = a1^C * s_c + e_c.  a1^C by repeated squaring in double.
 // ---------------------------------------------------------------------------------------------
-__global__ void spiir_chunk_carry_kernel(const float4* __restrict__ coef, const float2* __restrict__ state,
+__global__ void spiir_chunk_carry_kernel(const float4* __restrict__ coef, const float2* __restrict__ state, size_t sstride,
                                          float2* chunk_st, int nfilt /* G*F*32 */, int S, int NC, int C)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
@@ -381,7 +439,7 @@ __global__ void spiir_chunk_carry_kernel(const float4* __restrict__ coef, const 
     for (int s = 0; s < S; ++s) {
         float2* cs = chunk_st + (size_t)s * NC * nfilt + i;
         float2 cur = cs[0];                                // true end of chunk 0 = initial state of chunk 1
-        cs[0] = state[(size_t)s * nfilt + i];              // initial state of chunk 0
+        cs[0] = state[(size_t)s * sstride + i];            // initial state of chunk 0
         // the zero-state ends are fetched eight at a time so that their load latencies overlap
         for (int c0 = 1; c0 < NC; c0 += 8) {
             float2 ec[8];
@@ -403,15 +461,29 @@ __global__ void spiir_chunk_carry_kernel(const float4* __restrict__ coef, const 
 
 // state gather / scatter between plan order and the caller's [S][T][L] order
 __global__ void spiir_state_permute_kernel(float2* plan_state, float2* user_state, const int* __restrict__ pos,
-                                           int TL, int nfilt, int S, int to_user)
+                                           size_t TL, size_t nfilt, int S, int to_user)
 {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= TL) return;
     const int p = pos[i];
     for (int s = 0; s < S; ++s) {
         if (to_user) user_state[(size_t)s * TL + i] = plan_state[(size_t)s * nfilt + p];
         else plan_state[(size_t)s * nfilt + p] = user_state[(size_t)s * TL + i];
     }
+}
+
+// input history between the plan's ping-pong buffers ([S][Dpad], the newest sample last) and the caller's
+// [S][D] (the last D samples, oldest first)
+__global__ void spiir_hist_copy_kernel(float* const hbuf0, float* const hbuf1, const int* __restrict__ phase, float* user,
+                                       int S, int Dpad, int D, int to_user)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= S * Dpad) return;
+    const int s = i / Dpad, j = i % Dpad;
+    float* cur = (phase_read(phase) ? hbuf1 : hbuf0) + (size_t)s * Dpad;
+    const int k = j - (Dpad - D);                       // index in the caller's row
+    if (to_user) { if (k >= 0) user[(size_t)s * D + k] = cur[j]; }
+    else cur[j] = k >= 0 ? user[(size_t)s * D + k] : 0.f;
 }
 
 }  // namespace spiir

@@ -25,15 +25,18 @@ void set_error(const char* fmt, ...)
 
 const char* last_error() { return g_err; }
 
-// Filters per lane F and lanes per template LPT (power of two) with F*LPT >= L.
+// Filters per lane F, lanes per template LPT (power of two) and warps per template NP with F*LPT*NP >= L.
 //   L <= 4        : one lane per template (no cross-lane sum at all)
 //   5..31         : 2 / 4 / 8 lanes, 3-4 filters each
 //   32..512       : the 32 lanes of a warp, F = ceil(L/32) rounded up to an instantiated F
+//   513..2048     : NP = 2..8 adjacent warps of one CTA, F <= 8 each (a 513-filter template takes 544
+//                   threads of one block); the pair (NP, F) with the least padding wins, fewer warps on a tie
 static const int kFWarp[] = {1, 2, 3, 4, 5, 6, 7, 8, 10, 12, 14, 16};
 
-bool choose_lane_mapping(int L, int T, int* F, int* LPT)
+bool choose_lane_mapping(int L, int T, int* F, int* LPT, int* NP)
 {
-    if (L < 1) return false;
+    *NP = 1;
+    if (L < 1 || L > kMaxFiltersPerTemplate) return false;
     // 32..128 filters and enough templates to give every SM several warps anyway: half a warp per template
     // (two templates per warp).  The 16 outputs of a batch then cost a 16-lane butterfly for TWO templates,
     // i.e. half the shuffle / select work per update of the one-warp-per-template mapping.
@@ -42,10 +45,20 @@ bool choose_lane_mapping(int L, int T, int* F, int* LPT)
     if (L <= 8) { *LPT = 2; *F = (L + 1) / 2; return true; }
     if (L <= 16) { *LPT = 4; *F = (L + 3) / 4; return true; }
     if (L < 32) { *LPT = 8; *F = (L + 7) / 8; return true; }
-    int need = (L + 31) / 32;
-    for (int f : kFWarp)
-        if (f >= need) { *LPT = 32; *F = f; return true; }
-    return false;
+    *LPT = 32;
+    if (L <= 512) {
+        const int need = (L + 31) / 32;
+        for (int f : kFWarp)
+            if (f >= need) { *F = f; return true; }
+        return false;
+    }
+    int best = 1 << 30;
+    for (int np = 2; np <= 8; ++np) {
+        const int f = (L + 32 * np - 1) / (32 * np);
+        if (f > 8) continue;
+        if (f * 32 * np < best) { best = f * 32 * np; *F = f; *NP = np; }
+    }
+    return best < (1 << 30);
 }
 
 int lpt16_min_templates()
@@ -57,25 +70,29 @@ int lpt16_min_templates()
 
 static inline int bank_class(int d) { return ((d + 3) >> 2) & 7; }   // 16-byte bank group of W[Dpad + j - d]
 
-void build_layout(const spiir_c64* a1, const spiir_c64* b0, const int32_t* delays, int T, int L, int F, int LPT,
-                  bool avoid_conflicts, std::vector<float>* coef, std::vector<int32_t>* dly, std::vector<int32_t>* pos)
+void build_layout(const spiir_c64* a1, const spiir_c64* b0, const int32_t* delays, const int32_t* offsets, int L,
+                  const int32_t* templates, int T, int F, int LPT, int NP, bool avoid_conflicts,
+                  std::vector<float>* coef, std::vector<int32_t>* dly, int32_t* pos)
 {
     const int TPG = 32 / LPT;
-    const int G = (T + TPG - 1) / TPG;
+    const int G = LPT == 32 ? T * NP : (T + TPG - 1) / TPG;
     const size_t nf = (size_t)G * F * 32;
+    const int slots = NP * F * LPT;                        // filter places of one template
     coef->assign(nf * 4, 0.f);
     dly->assign(nf, 0);
-    pos->assign((size_t)T * L, -1);
-    std::vector<int> order;   // order[k] = filter placed at (slot, lane) position k of the template, or -1
-    for (int t = 0; t < T; ++t) {
-        const int32_t* d = delays + (size_t)t * L;
-        order.assign((size_t)F * LPT, -1);
+    std::vector<int> order;   // order[k] = filter (index within the template) placed at place k = (piece, slot, lane), or -1
+    for (int tc = 0; tc < T; ++tc) {
+        const int t = templates ? templates[tc] : tc;
+        const size_t base = offsets ? (size_t)offsets[t] : (size_t)t * L;
+        const int Lt = offsets ? offsets[t + 1] - offsets[t] : L;
+        const int32_t* d = delays + base;
+        order.assign((size_t)slots, -1);
         if (avoid_conflicts && LPT >= 8) {
             // groups of 8 lanes (one quarter warp, one slot) should see 8 distinct bank classes
             std::vector<int> bucket[8];
-            for (int l = L - 1; l >= 0; --l) bucket[bank_class(d[l])].push_back(l);
-            const int ngroups = F * LPT / 8;
-            int left = L;
+            for (int l = Lt - 1; l >= 0; --l) bucket[bank_class(d[l])].push_back(l);
+            const int ngroups = slots / 8;
+            int left = Lt;
             for (int gi = 0; gi < ngroups && left > 0; ++gi) {
                 bool used[8] = {false, false, false, false, false, false, false, false};
                 for (int r = 0; r < 8 && left > 0; ++r) {
@@ -89,26 +106,26 @@ void build_layout(const spiir_c64* a1, const spiir_c64* b0, const int32_t* delay
                     const int l = bucket[best].back();
                     bucket[best].pop_back();
                     --left;
-                    const int f = gi / (LPT / 8), q = gi % (LPT / 8);
-                    order[(size_t)f * LPT + q * 8 + r] = l;
+                    order[(size_t)gi * 8 + r] = l;         // place = (piece, slot, quarter) * 8 + r: slot-major inside a piece
                 }
             }
         } else {
-            for (int l = 0; l < L; ++l) order[(size_t)(l / LPT) * LPT + (l % LPT)] = l;
+            for (int l = 0; l < Lt; ++l) order[(size_t)l] = l;
         }
-        const int g = t / TPG, lane0 = (t % TPG) * LPT;
-        for (int f = 0; f < F; ++f)
-            for (int j = 0; j < LPT; ++j) {
-                const int l = order[(size_t)f * LPT + j];
-                if (l < 0) continue;
-                const size_t idx = ((size_t)g * F + f) * 32 + lane0 + j;
-                (*coef)[idx * 4 + 0] = a1[(size_t)t * L + l].re;
-                (*coef)[idx * 4 + 1] = a1[(size_t)t * L + l].im;
-                (*coef)[idx * 4 + 2] = b0[(size_t)t * L + l].re;
-                (*coef)[idx * 4 + 3] = b0[(size_t)t * L + l].im;
-                (*dly)[idx] = d[l];
-                (*pos)[(size_t)t * L + l] = (int32_t)idx;
-            }
+        for (int k = 0; k < slots; ++k) {
+            const int l = order[(size_t)k];
+            if (l < 0) continue;
+            const int piece = k / (F * LPT), f = (k % (F * LPT)) / LPT, j = k % LPT;
+            const int g = LPT == 32 ? tc * NP + piece : tc / TPG;
+            const int lane0 = LPT == 32 ? 0 : (tc % TPG) * LPT;
+            const size_t idx = ((size_t)g * F + f) * 32 + lane0 + j;
+            (*coef)[idx * 4 + 0] = a1[base + l].re;
+            (*coef)[idx * 4 + 1] = a1[base + l].im;
+            (*coef)[idx * 4 + 2] = b0[base + l].re;
+            (*coef)[idx * 4 + 3] = b0[base + l].im;
+            (*dly)[idx] = d[l];
+            if (pos) pos[base + l] = (int32_t)idx;
+        }
     }
 }
 
@@ -140,13 +157,14 @@ spiir_status compute_geometry(int T, int L, int S, int Dpad, int n, int opt_chun
                               int smem_optin, FilterGeometry* g)
 {
     memset(g, 0, sizeof *g);
-    if (!choose_lane_mapping(L, T, &g->F, &g->LPT)) {
-        set_error("n_filters = %d is not supported (1..512)", L);
+    if (!choose_lane_mapping(L, T, &g->F, &g->LPT, &g->NP)) {
+        set_error("n_filters = %d is not supported (1..%d)", L, kMaxFiltersPerTemplate);
         return SPIIR_EUNSUPPORTED;
     }
     g->TPG = 32 / g->LPT;
-    g->G = (T + g->TPG - 1) / g->TPG;
+    g->G = g->LPT == 32 ? T * g->NP : (T + g->TPG - 1) / g->TPG;
     const int kBatch = 16, kMaxWarps = 8;
+    const int kRedWarpBytes = (32 * 9 + 64) * 16;          // spiir_filter.cuh: kRedWarp4 float4 per warp (LPT = 32)
     // time chunks: only when the bank alone cannot fill the machine
     int NC = 1;
     const long tasks = (long)S * g->G;
@@ -172,8 +190,14 @@ spiir_status compute_geometry(int T, int L, int S, int Dpad, int n, int opt_chun
     NC = (n + C - 1) / C;
     if (NC <= 1) { NC = 1; C = round_up(std::max(n, 1), kBatch); }
     g->NC = NC; g->C = C;
+    const long W = tasks * NC;
+    int warps = (int)std::min<long>(kMaxWarps, std::max<long>(1, (W + n_sm - 1) / n_sm));
+    warps = std::min(warps, g->G);
+    if (g->NP > 1) warps = std::max(g->NP, warps / g->NP * g->NP);      // the warps of a template share a CTA
+    g->warps = warps;
+    const int red_bytes = g->LPT == 32 ? warps * kRedWarpBytes : 0;
     // time tile: as long as shared memory allows (4 shifted copies of Dpad + NT + 32 floats)
-    const int budget_floats = (smem_optin - 64) / 16;
+    const int budget_floats = (smem_optin - 64 - red_bytes) / 16;
     int NT = C;
     if (Dpad + NT + 32 > budget_floats) NT = (budget_floats - Dpad - 32) / kBatch * kBatch;
     if (NT < kBatch) {
@@ -182,11 +206,7 @@ spiir_status compute_geometry(int T, int L, int S, int Dpad, int n, int opt_chun
     }
     g->NT = NT;
     g->CS = Dpad + NT + 32;
-    g->smem_bytes = 16 * g->CS + 16;
-    const long W = tasks * NC;
-    int warps = (int)std::min<long>(kMaxWarps, std::max<long>(1, (W + n_sm - 1) / n_sm));
-    warps = std::min(warps, g->G);
-    g->warps = warps;
+    g->smem_bytes = 16 * g->CS + 16 + red_bytes;
     int gx = (g->G + warps - 1) / warps;
     const int resident = std::max(1, (2 * n_sm) / (S * NC));   // CTAs per (stream, chunk) kept resident
     if (gx > resident && (long)gx * S * NC > 2L * n_sm) gx = resident;
@@ -238,7 +258,7 @@ spiir_status kaiser_taps(int n_taps, double beta, double cutoff, float* out)
 extern "C" {
 
 const char* spiir_last_error(void) { return spiir::last_error(); }
-const char* spiir_version(void) { return "spiir-b200 0.1 sm_100a"; }
+const char* spiir_version(void) { return "spiir-b200 0.2 sm_100a"; }
 
 spiir_status spiir_kaiser_taps(int n_taps, double kaiser_beta, double cutoff, float* taps_out)
 {
@@ -249,15 +269,16 @@ spiir_status spiir_host_layout(const spiir_c64* a1, const spiir_c64* b0, const i
                                int n_filters, int avoid_conflicts, int32_t* pos_out, float* coef_out,
                                int32_t* dly_out, int info[4], double* conflict_degree)
 {
-    int F, LPT;
-    if (!a1 || !b0 || !delays || n_templates < 1 || !spiir::choose_lane_mapping(n_filters, n_templates, &F, &LPT)) {
+    int F, LPT, NP;
+    if (!a1 || !b0 || !delays || n_templates < 1 || !spiir::choose_lane_mapping(n_filters, n_templates, &F, &LPT, &NP)) {
         spiir::set_error("spiir_host_layout: bad arguments");
         return SPIIR_EINVAL;
     }
     std::vector<float> coef;
-    std::vector<int32_t> dly, pos;
-    spiir::build_layout(a1, b0, delays, n_templates, n_filters, F, LPT, avoid_conflicts != 0, &coef, &dly, &pos);
-    const int TPG = 32 / LPT, G = (n_templates + TPG - 1) / TPG;
+    std::vector<int32_t> dly, pos((size_t)n_templates * n_filters, -1);
+    spiir::build_layout(a1, b0, delays, nullptr, n_filters, nullptr, n_templates, F, LPT, NP, avoid_conflicts != 0, &coef, &dly,
+                        pos.data());
+    const int TPG = 32 / LPT, G = LPT == 32 ? n_templates * NP : (n_templates + TPG - 1) / TPG;
     if (info) { info[0] = F; info[1] = LPT; info[2] = G; info[3] = (int)(dly.size()); }
     if (pos_out) memcpy(pos_out, pos.data(), pos.size() * sizeof(int32_t));
     if (coef_out) memcpy(coef_out, coef.data(), coef.size() * sizeof(float));
@@ -280,6 +301,43 @@ spiir_status spiir_host_geometry(int n_templates, int n_filters, int n_streams, 
     if (st != SPIIR_OK) return st;
     info[0] = g.F; info[1] = g.LPT; info[2] = g.warps; info[3] = g.grid_x * g.grid_y;
     info[4] = g.NC; info[5] = g.smem_bytes; info[6] = g.NT; info[7] = g.launches;
+    return SPIIR_OK;
+}
+
+spiir_status spiir_host_lane_mapping(int n_filters, int n_templates, int info[3])
+{
+    int F, LPT, NP;
+    if (!info || n_templates < 1 || !spiir::choose_lane_mapping(n_filters, n_templates, &F, &LPT, &NP)) {
+        spiir::set_error("spiir_host_lane_mapping: n_filters = %d not supported (1..%d)", n_filters, spiir::kMaxFiltersPerTemplate);
+        return SPIIR_EUNSUPPORTED;
+    }
+    info[0] = F; info[1] = LPT; info[2] = NP;
+    return SPIIR_OK;
+}
+
+// PAPER.md:79, reading R8 (see include/spiir.h).
+spiir_status spiir_assign_rates(const spiir_c64* a1, int n, int base_rate_hz, const int* rates_hz, int n_rates,
+                                double band_factor, int32_t* rate_index_out)
+{
+    if (!a1 || !rates_hz || !rate_index_out || n < 0 || n_rates < 1 || base_rate_hz < 1 || rates_hz[0] != base_rate_hz ||
+        !(band_factor >= 0.0)) {
+        spiir::set_error("spiir_assign_rates: bad arguments");
+        return SPIIR_EINVAL;
+    }
+    for (int h = 1; h < n_rates; ++h)
+        if (rates_hz[h] >= rates_hz[h - 1] || rates_hz[h] < 1) { spiir::set_error("spiir_assign_rates: rates must descend"); return SPIIR_EINVAL; }
+    for (int i = 0; i < n; ++i) {
+        const double re = a1[i].re, im = a1[i].im, mag = hypot(re, im);
+        int pick = 0;
+        if (mag > 0.0 && mag < 1.0) {
+            const double f0 = fabs(atan2(im, re)) * base_rate_hz / (2.0 * M_PI);
+            const double df = -log(mag) * base_rate_hz / (2.0 * M_PI);
+            const double nyq = 2.0 * (f0 + band_factor * df);
+            for (int h = n_rates - 1; h >= 0; --h)
+                if ((double)rates_hz[h] >= nyq) { pick = h; break; }     // lowest available rate that still holds the band
+        }
+        rate_index_out[i] = pick;
+    }
     return SPIIR_OK;
 }
 

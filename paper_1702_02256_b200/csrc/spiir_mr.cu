@@ -4,7 +4,6 @@
 // Every stage keeps its own streaming history, so consecutive calls continue one stream.
 #include <algorithm>
 #include <stdio.h>
-#include <time.h>
 #include <new>
 #include <vector>
 
@@ -23,6 +22,7 @@ struct spiir_mr_plan {
     std::vector<cudaStream_t> side;         // [H]
     std::vector<cudaEvent_t> ev_bank;       // [H]
     cudaEvent_t ev_start = nullptr, ev_chain = nullptr;
+    spiir::Arena arena;                     // every device byte of the plan (caller's workspace or one library block)
 };
 
 using namespace spiir;
@@ -35,13 +35,51 @@ void spiir_mr_plan_destroy(spiir_mr_plan_t* p)
     for (auto b : p->banks) spiir_plan_destroy(b);
     for (auto r : p->downs) spiir_resamp_destroy(r);
     for (auto r : p->ups) spiir_resamp_destroy(r);
-    for (auto q : p->d_x) cudaFree(q);
-    for (auto q : p->d_z) cudaFree(q);
     for (auto q : p->side) if (q) cudaStreamDestroy(q);
     for (auto q : p->ev_bank) if (q) cudaEventDestroy(q);
     if (p->ev_start) cudaEventDestroy(p->ev_start);
     if (p->ev_chain) cudaEventDestroy(p->ev_chain);
+    spiir::arena_close(&p->arena);
     delete p;
+}
+
+static const spiir_mr_opts kMrDefaults = {1, 0, 192, 5.0, 0.25, 192, 5.0, 0.25, nullptr, 0};
+
+static bool mr_opts_ok(const spiir_mr_opts& o, int n_rates)
+{
+    return o.n_streams >= 1 && o.max_block >= 1 && (o.max_block % (1 << (n_rates - 1))) == 0;
+}
+
+// device bytes of a multirate plan: the banks, the stages, the per-rate strain and SNR scratch
+static size_t mr_measure(int n_rates, const int* n_filters_per_rate, const int* max_delay_per_rate, int n_templates,
+                         const spiir_mr_opts& o)
+{
+    Arena a;
+    for (int h = 0; h < n_rates; ++h) {
+        const int nb = o.max_block >> h;
+        const size_t bank = spiir_plan_workspace_bytes(n_templates, n_filters_per_rate[h], max_delay_per_rate[h], o.n_streams, nb, 0);
+        if (!bank) return 0;
+        a.take(bank);
+        if (h > 0) {
+            const size_t dn = spiir_resamp_workspace_bytes(SPIIR_DOWN2, o.n_taps_down, o.n_streams);
+            const size_t up = spiir_resamp_workspace_bytes(SPIIR_UP2, o.n_taps_up, o.n_streams * n_templates);
+            if (!dn || !up) return 0;
+            a.take(dn); a.take(up);
+            a.take((size_t)o.n_streams * nb * sizeof(float));
+            a.take((size_t)o.n_streams * n_templates * nb * sizeof(spiir_c64));
+        }
+    }
+    return (a.used + 255) & ~(size_t)255;
+}
+
+size_t spiir_mr_workspace_bytes(int n_rates, const int* n_filters_per_rate, const int* max_delay_per_rate, int n_templates,
+                                const spiir_mr_opts* opts)
+{
+    if (n_rates < 1 || n_rates > 16 || !n_filters_per_rate || !max_delay_per_rate || n_templates < 1 || !opts || !mr_opts_ok(*opts, n_rates)) {
+        set_error("spiir_mr_workspace_bytes: bad arguments (options with max_block are required)");
+        return 0;
+    }
+    return mr_measure(n_rates, n_filters_per_rate, max_delay_per_rate, n_templates, *opts);
 }
 
 spiir_status spiir_mr_plan_create(spiir_mr_plan_t** out, int n_rates, const int* rates_hz, const spiir_c64* const* a1,
@@ -59,38 +97,50 @@ spiir_status spiir_mr_plan_create(spiir_mr_plan_t** out, int n_rates, const int*
             set_error("spiir_mr_plan_create: rates must halve (rate[%d] = %d, rate[%d] = %d)", h - 1, rates_hz[h - 1], h, rates_hz[h]);
             return SPIIR_EINVAL;
         }
-    spiir_mr_opts o = {1, rates_hz[0], 192, 5.0, 0.25};
+    spiir_mr_opts o = kMrDefaults;
+    o.max_block = rates_hz[0];
     if (opts) o = *opts;
-    if (o.n_streams < 1 || o.max_block < 1 || (o.max_block % (1 << (n_rates - 1))) != 0) {
+    if (!mr_opts_ok(o, n_rates)) {
         set_error("spiir_mr_plan_create: max_block must be a positive multiple of 2^(n_rates-1)");
         return SPIIR_EINVAL;
     }
+    std::vector<int> dmax(n_rates, 0);
+    for (int h = 0; h < n_rates; ++h) {
+        if (!a1[h] || !b0[h] || !delays[h] || n_filters_per_rate[h] < 1) { set_error("spiir_mr_plan_create: bad bank %d", h); return SPIIR_EINVAL; }
+        const size_t TL = (size_t)n_templates * n_filters_per_rate[h];
+        for (size_t i = 0; i < TL; ++i) {
+            if (delays[h][i] < 0 || delays[h][i] >= (1 << 20)) { set_error("spiir_mr_plan_create: delay out of range (rate %d)", h); return SPIIR_EINVAL; }
+            dmax[h] = std::max(dmax[h], (int)delays[h][i]);
+        }
+    }
+    const size_t need = mr_measure(n_rates, n_filters_per_rate, dmax.data(), n_templates, o);
+    if (!need) return SPIIR_EUNSUPPORTED;
     spiir_mr_plan* p = new (std::nothrow) spiir_mr_plan;
     if (!p) return SPIIR_ENOMEM;
+    spiir_status rc = arena_open(&p->arena, o.workspace, o.workspace_bytes, need, "spiir_mr_plan_create");
+    if (rc != SPIIR_OK) { delete p; return rc; }
     p->H = n_rates; p->T = n_templates; p->S = o.n_streams; p->max_block = o.max_block;
     p->rates.assign(rates_hz, rates_hz + n_rates);
     p->d_x.assign(n_rates, nullptr);
     p->d_z.assign(n_rates, nullptr);
-    spiir_status rc = SPIIR_OK;
     for (int h = 0; h < n_rates && rc == SPIIR_OK; ++h) {
         const int nb = o.max_block >> h;
-        spiir_plan_opts po = {o.n_streams, nb, 0, 0};
+        spiir_plan_opts po = {o.n_streams, nb, 0, 0, nullptr, 0};
         spiir_plan_t* b = nullptr;
-        rc = spiir_plan_create(&b, a1[h], b0[h], delays[h], n_templates, n_filters_per_rate[h], rates_hz[h], &po);
+        rc = plan_create_in(&b, a1[h], b0[h], delays[h], nullptr, n_templates, n_filters_per_rate[h], rates_hz[h], po, &p->arena);
         if (rc != SPIIR_OK) break;
         p->banks.push_back(b);
         if (h > 0) {
             spiir_resamp_t* d = nullptr;
-            rc = spiir_resamp_create(&d, SPIIR_DOWN2, o.n_taps, o.kaiser_beta, o.cutoff, o.n_streams, nb * 2);
+            rc = resamp_create_in(&d, SPIIR_DOWN2, o.n_taps_down, o.kaiser_beta_down, o.cutoff_down, o.n_streams, nb * 2, &p->arena);
             if (rc != SPIIR_OK) break;
             p->downs.push_back(d);
             spiir_resamp_t* u = nullptr;
-            rc = spiir_resamp_create(&u, SPIIR_UP2, o.n_taps, o.kaiser_beta, o.cutoff, o.n_streams * n_templates, nb);
+            rc = resamp_create_in(&u, SPIIR_UP2, o.n_taps_up, o.kaiser_beta_up, o.cutoff_up, o.n_streams * n_templates, nb, &p->arena);
             if (rc != SPIIR_OK) break;
             p->ups.push_back(u);
-            cudaError_t e = cudaMalloc(&p->d_x[h], (size_t)o.n_streams * nb * sizeof(float));
-            if (e == cudaSuccess) e = cudaMalloc(&p->d_z[h], (size_t)o.n_streams * n_templates * nb * sizeof(spiir_c64));
-            if (e != cudaSuccess) { rc = cuda_fail(e, "spiir_mr_plan_create scratch"); break; }
+            p->d_x[h] = p->arena.take_n<float>((size_t)o.n_streams * nb);
+            p->d_z[h] = p->arena.take_n<spiir_c64>((size_t)o.n_streams * n_templates * nb);
         }
     }
     if (rc == SPIIR_OK && n_rates > 1) {
@@ -137,11 +187,6 @@ spiir_status spiir_mr_filter(spiir_mr_plan_t* p, const float* x, int n, spiir_c6
         }
     } else if (rc != SPIIR_OK) return rc;
     SPIIR_CUDA(cudaEventRecord(p->ev_chain, st));
-#ifdef MR_TRACE
-    static double tr[4]; static int ntr = 0;
-    auto now = []() { timespec ts; clock_gettime(CLOCK_MONOTONIC, &ts); return ts.tv_sec * 1e6 + ts.tv_nsec * 1e-3; };
-    cudaDeviceSynchronize(); double t1 = now();
-#endif
     // row a9: per-rate banks, side by side.  Unchunked banks that share a lane mapping go out as ONE launch
     // (the low rates are a few microseconds of work each); everything else gets its own side stream.
     std::vector<char> done(p->H, 0), rec(p->H, 0);
@@ -149,13 +194,13 @@ spiir_status spiir_mr_filter(spiir_mr_plan_t* p, const float* x, int n, spiir_c6
     for (int h = 1; h < p->H; ++h) {
         if (done[h]) continue;
         FilterGeometry gh;
-        if ((rc = plan_geometry(p->banks[h], n >> h, &gh)) != SPIIR_OK) return rc;
+        if ((rc = plan_geometry(p->banks[h], p->banks[h]->cls[0], n >> h, &gh)) != SPIIR_OK) return rc;
         std::vector<int> grp(1, h);
-        if (gh.NC == 1)
+        if (gh.NC == 1 && gh.NP == 1)
             for (int j = h + 1; j < p->H && (int)grp.size() < 8; ++j) {
                 FilterGeometry gj;
-                if (done[j] || plan_geometry(p->banks[j], n >> j, &gj) != SPIIR_OK) continue;
-                if (gj.NC == 1 && gj.F == gh.F && gj.LPT == gh.LPT) grp.push_back(j);
+                if (done[j] || plan_geometry(p->banks[j], p->banks[j]->cls[0], n >> j, &gj) != SPIIR_OK) continue;
+                if (gj.NC == 1 && gj.NP == 1 && gj.F == gh.F && gj.LPT == gh.LPT) grp.push_back(j);
             }
         SPIIR_CUDA(cudaStreamWaitEvent(p->side[h], p->ev_chain, 0));
         rc = SPIIR_EUNSUPPORTED;
@@ -176,9 +221,6 @@ spiir_status spiir_mr_filter(spiir_mr_plan_t* p, const float* x, int n, spiir_c6
     }
     for (int h = 0; h < p->H; ++h)                                                         // join
         if (rec[h]) SPIIR_CUDA(cudaStreamWaitEvent(st, p->ev_bank[h], 0));
-#ifdef MR_TRACE
-    cudaDeviceSynchronize(); double t2 = now();
-#endif
     // row a10: up + accumulate cascade, lowest rate first; one launch when the tap count has a fused kernel
     {
         const int nst = p->H - 1;
@@ -197,11 +239,6 @@ spiir_status spiir_mr_filter(spiir_mr_plan_t* p, const float* x, int n, spiir_c6
             }
         } else if (rc != SPIIR_OK) return rc;
     }
-#ifdef MR_TRACE
-    cudaDeviceSynchronize(); double t3 = now();
-    tr[1] += t2 - t1; tr[2] += t3 - t2; ++ntr;
-    if (ntr % 20 == 0) { fprintf(stderr, "MR_TRACE banks1..H-1 %.1f us  up chain %.1f us (avg of 20)\n", tr[1] / 20, tr[2] / 20); tr[1] = tr[2] = 0; }
-#endif
     return SPIIR_OK;
 }
 
@@ -212,6 +249,53 @@ spiir_status spiir_mr_plan_reset(spiir_mr_plan_t* p, void* cuda_stream)
     for (auto b : p->banks) if ((rc = spiir_plan_reset(b, cuda_stream)) != SPIIR_OK) return rc;
     for (auto r : p->downs) if ((rc = spiir_resamp_reset(r, cuda_stream)) != SPIIR_OK) return rc;
     for (auto r : p->ups) if ((rc = spiir_resamp_reset(r, cuda_stream)) != SPIIR_OK) return rc;
+    return rc;
+}
+
+// Resume state blob (layout in include/spiir.h): sections in a fixed order, each 16-byte aligned.
+static size_t mr_state_walk(spiir_mr_plan_t* p, char* blob, int to_user, cudaStream_t st, spiir_status* rc)
+{
+    size_t off = 0;
+    auto section = [&](size_t bytes) { const size_t at = off; off = (off + bytes + 15) & ~(size_t)15; return at; };
+    *rc = SPIIR_OK;
+    for (int h = 0; h < p->H && *rc == SPIIR_OK; ++h) {
+        spiir_plan* b = p->banks[h];
+        const size_t ay = section((size_t)b->S * b->n_filters_total * sizeof(spiir_c64));
+        const size_t ah = section((size_t)b->S * b->Dmax * sizeof(float));
+        if (blob) *rc = plan_state_copy(b, reinterpret_cast<spiir_c64*>(blob + ay), b->Dmax ? reinterpret_cast<float*>(blob + ah) : nullptr,
+                                        to_user, st);
+    }
+    for (size_t k = 0; k < p->downs.size() && *rc == SPIIR_OK; ++k) {
+        const size_t at = section((size_t)p->downs[k]->rows * p->downs[k]->H * sizeof(float));
+        if (blob) *rc = resamp_state_copy(p->downs[k], blob + at, to_user, st);
+    }
+    for (size_t k = 0; k < p->ups.size() && *rc == SPIIR_OK; ++k) {
+        const size_t at = section((size_t)p->ups[k]->rows * p->ups[k]->H * sizeof(spiir_c64));
+        if (blob) *rc = resamp_state_copy(p->ups[k], blob + at, to_user, st);
+    }
+    return off;
+}
+
+size_t spiir_mr_plan_state_bytes(const spiir_mr_plan_t* p)
+{
+    if (!p) return 0;
+    spiir_status rc;
+    return mr_state_walk(const_cast<spiir_mr_plan_t*>(p), nullptr, 1, nullptr, &rc);
+}
+
+spiir_status spiir_mr_plan_get_state(spiir_mr_plan_t* p, void* blob_out, void* cuda_stream)
+{
+    if (!p || !blob_out || (reinterpret_cast<uintptr_t>(blob_out) & 15u)) { set_error("spiir_mr_plan_get_state: NULL or misaligned blob"); return SPIIR_EINVAL; }
+    spiir_status rc;
+    mr_state_walk(p, static_cast<char*>(blob_out), 1, static_cast<cudaStream_t>(cuda_stream), &rc);
+    return rc;
+}
+
+spiir_status spiir_mr_plan_set_state(spiir_mr_plan_t* p, const void* blob_in, void* cuda_stream)
+{
+    if (!p || !blob_in || (reinterpret_cast<uintptr_t>(blob_in) & 15u)) { set_error("spiir_mr_plan_set_state: NULL or misaligned blob"); return SPIIR_EINVAL; }
+    spiir_status rc;
+    mr_state_walk(p, static_cast<char*>(const_cast<void*>(blob_in)), 0, static_cast<cudaStream_t>(cuda_stream), &rc);
     return rc;
 }
 
@@ -228,17 +312,17 @@ int spiir_mr_launches(const spiir_mr_plan_t* p, int n)
     }
     std::vector<FilterGeometry> g(p->H);
     for (int h = 0; h < p->H; ++h)
-        if (plan_geometry(p->banks[h], std::max(1, n >> h), &g[h]) != SPIIR_OK) return 0;
+        if (plan_geometry(p->banks[h], p->banks[h]->cls[0], std::max(1, n >> h), &g[h]) != SPIIR_OK) return 0;
     std::vector<char> done(p->H, 0);
     for (int h = 0; h < p->H; ++h) {
         if (done[h]) continue;
-        total += g[h].launches;
+        total += plan_launches(p->banks[h], std::max(1, n >> h));
         done[h] = 1;
         // the same grouping as spiir_mr_filter: unchunked banks h >= 1 with one warp per template and F <= 8
-        if (h >= 1 && g[h].NC == 1 && g[h].LPT == 32 && g[h].F <= 8) {
+        if (h >= 1 && g[h].NC == 1 && g[h].NP == 1 && g[h].LPT == 32 && g[h].F <= 8) {
             int members = 1;
             for (int j = h + 1; j < p->H && members < 8; ++j)
-                if (!done[j] && g[j].NC == 1 && g[j].F == g[h].F && g[j].LPT == g[h].LPT) { done[j] = 1; ++members; }
+                if (!done[j] && g[j].NC == 1 && g[j].NP == 1 && g[j].F == g[h].F && g[j].LPT == g[h].LPT) { done[j] = 1; ++members; }
         }
     }
     return total;

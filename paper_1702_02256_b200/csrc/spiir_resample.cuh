@@ -10,7 +10,7 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
-#include "spiir_filter.cuh"   // phase_read / last_cta_arrives
+#include "spiir_common.cuh"   // phase_read / last_cta_arrives
 
 namespace spiir {
 

@@ -40,3 +40,31 @@ def stream_gpu_plan(plan, blocks):
 
 def stream_oracle(orc, blocks):
     return np.concatenate([orc.filter(x) for x in blocks], axis=-1)
+
+
+class ParityAccumulator:
+    """The two error measures of F10 over a run that is compared block by block (full banks do not fit in
+    host memory as one concatenated complex128 array): per (stream, template) sums of |dz|^2 and |z_ref|^2 and
+    running maxima of |dz| and |z_ref| over the whole run."""
+
+    def __init__(self):
+        self.num = self.den = self.mx = self.mref = None
+
+    def add(self, z, ref):
+        z = np.asarray(z).reshape(ref.shape)
+        d = np.abs(z - ref)
+        r = np.abs(ref)
+        num, den, mx, mref = (d ** 2).sum(-1), (r ** 2).sum(-1), d.max(-1), r.max(-1)
+        if self.num is None:
+            self.num, self.den, self.mx, self.mref = num, den, mx, mref
+        else:
+            self.num += num; self.den += den
+            self.mx = np.maximum(self.mx, mx); self.mref = np.maximum(self.mref, mref)
+
+    def check(self, what=""):
+        rel = np.sqrt(self.num / np.where(self.den > 0, self.den, 1.0))
+        mab = self.mx / np.where(self.mref > 0, self.mref, 1.0)
+        assert np.all(self.den > 0), f"{what}: a reference series is identically zero"
+        assert rel.max() <= REL_L2_TOL, f"{what}: rel-L2 {rel.max():.3e} > {REL_L2_TOL} (template {np.unravel_index(rel.argmax(), rel.shape)})"
+        assert mab.max() <= MAX_ABS_TOL, f"{what}: max-abs ratio {mab.max():.3e} > {MAX_ABS_TOL}"
+        return float(rel.max()), float(mab.max())

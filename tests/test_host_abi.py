@@ -57,7 +57,7 @@ def test_argument_errors_need_no_gpu(sp):
     d = np.array([[0, 1, -1, 2]], np.int32)
     assert L.spiir_plan_create(ctypes.byref(h), a.ctypes.data, a.ctypes.data, d.ctypes.data, 1, 4, 4096, None) == sp.SPIIR_EINVAL
     assert L.spiir_filter(None, None, 16, None, None) == sp.SPIIR_EINVAL
-    assert L.spiir_resamp_create(ctypes.byref(h), 0, 191, 5.0, 0.25, 1, 64) == sp.SPIIR_EINVAL     # odd tap count
+    assert L.spiir_resamp_create(ctypes.byref(h), 0, 191, 5.0, 0.25, 1, None) == sp.SPIIR_EINVAL   # odd tap count
     assert L.spiir_resample_down(None, None, 2, None, None) == sp.SPIIR_EINVAL
     rates = (ctypes.c_int * 2)(4096, 1024)
     assert L.spiir_mr_plan_create(ctypes.byref(h), 2, rates, ctypes.byref(h), ctypes.byref(h), ctypes.byref(h),
@@ -81,6 +81,49 @@ def test_lane_mapping(sp, L, F, LPT):
     g = sp.spiir_host_geometry(64, L, 1, 100, 1024)
     assert (g["F"], g["lanes_per_template"]) == (F, LPT)
     assert F * LPT >= L
+
+
+@pytest.mark.parametrize("L,F,NP", [(513, 6, 3), (544, 6, 3), (600, 5, 4), (1024, 8, 4), (1025, 7, 5), (2048, 8, 8)])
+def test_lane_mapping_multi_warp_templates(sp, L, F, NP):
+    """a 513-filter template takes 544 threads of one block; here it spans NP warps of one CTA with
+    F filters per lane, the pair with the least padding."""
+    m = sp.spiir_host_lane_mapping(L)
+    assert (m["F"], m["lanes_per_template"], m["warps_per_template"]) == (F, 32, NP)
+    assert F * 32 * NP >= L and F <= 8
+    g = sp.spiir_host_geometry(64, L, 1, 100, 1024)
+    assert g["warps_per_cta"] % NP == 0 and g["warps_per_cta"] <= 8
+    with pytest.raises(sp.SpiirError):
+        sp.spiir_host_lane_mapping(2049)
+    with pytest.raises(sp.SpiirError):
+        sp.spiir_host_geometry(4, 2049, 1, 10, 256)
+
+
+def test_rate_assignment_reading_r8(sp):
+    """PAPER.md:79 / DESIGN.md reading R8: lowest available rate whose Nyquist band holds f0 + band_factor * df."""
+    rates = [4096, 2048, 1024, 512, 256, 128, 64]
+    # |a1| close to 1: negligible bandwidth term; centre frequencies just below / above each rate's Nyquist frequency
+    f0 = np.array([10.0, 31.9, 32.1, 63.0, 65.0, 500.0, 513.0, 1023.0, 1025.0, 2047.0])
+    a1 = (0.99999 * np.exp(2j * np.pi * f0 / 4096)).astype(np.complex64)          # df = 0.0065 Hz
+    idx = sp.spiir_assign_rates(a1, 4096, rates, band_factor=1.0)
+    want = [6, 6, 5, 5, 4, 2, 1, 1, 0, 0]
+    assert idx.tolist() == want
+    # negative frequencies count by magnitude; a strongly damped filter is wide and moves up
+    a = np.array([0.999 * np.exp(-2j * np.pi * 100 / 4096), 0.5 * np.exp(2j * np.pi * 100 / 4096)], np.complex64)
+    i2 = sp.spiir_assign_rates(a, 4096, rates, band_factor=1.0)
+    assert i2[0] == 4 and i2[1] < i2[0]
+    assert sp.spiir_assign_rates(a, 4096, rates, band_factor=0.0).tolist() == [4, 4]
+    with pytest.raises(sp.SpiirError):
+        sp.spiir_assign_rates(a, 4096, [2048, 1024])          # rates[0] must be the base rate
+
+
+def test_workspace_queries_fail_loudly_without_a_device(sp):
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a GPU is present")
+    assert sp.lib().spiir_plan_workspace_bytes(16, 128, 2047, 1, 4096, 0) == 0
+    assert b"CUDA" in sp.lib().spiir_last_error()
+    assert sp.lib().spiir_resamp_workspace_bytes(0, 192, 3) > 0          # stage sizes need no device
+    assert sp.lib().spiir_resamp_workspace_bytes(0, 191, 3) == 0
 
 
 def test_chunking_follows_the_cost_model(sp):
@@ -148,11 +191,13 @@ def test_geometry_of_the_baseline_configs(sp):
     assert g1["time_chunks"] == 1 and g1["launches"] == 1
     assert g1["warps_per_cta"] == 7 and g1["grid"] == 147                       # one CTA per SM, 7 templates each
     assert g1["time_tile"] == 4096 and g1["smem_bytes"] <= 232448
+    assert g1["smem_bytes"] == 16 * (4096 + 4096 + 32) + 16 + 7 * (32 * 9 + 64) * 16     # window copies + reduction tiles
     g0 = sp.spiir_host_geometry(16, 128, 1, 2047, 4096)
     assert g0["time_chunks"] > 8 and g0["launches"] == 3                        # 16 warps of work -> chunked scan
     g4 = sp.spiir_host_geometry(16384, 256, 2, 2047, 2048)
     assert g4["time_chunks"] == 1 and g4["warps_per_cta"] == 8
     assert g4["grid"] <= 2 * 148 + 2                                            # persistent CTAs loop over groups
+    assert 2 * (g4["smem_bytes"] + 1024) <= 233472                              # two CTAs share an SM
     # forcing chunks / forbidding them
     assert sp.spiir_host_geometry(1024, 256, 1, 4095, 4096, time_chunks=4)["time_chunks"] == 4
     assert sp.spiir_host_geometry(16, 128, 1, 2047, 4096, time_chunks=1)["time_chunks"] == 1
