@@ -102,8 +102,24 @@ static filter_kernel_t pick_small(int F, bool noz)
     return nullptr;
 }
 
-static filter_kernel_t pick_kernel(int F, int LPT, bool noz)
+template <int F>
+static filter_kernel_t pick_multi_warp(bool noz)
 {
+    return noz ? (filter_kernel_t)spiir_filter_kernel<F, 32, true, true> : (filter_kernel_t)spiir_filter_kernel<F, 32, false, true>;
+}
+
+static filter_kernel_t pick_kernel(int F, int LPT, int NP, bool noz)
+{
+    if (NP > 1) {                                         // templates of more than 512 filters: NP warps x F <= 8
+        if (LPT != 32) return nullptr;
+        switch (F) {
+            case 5: return pick_multi_warp<5>(noz);
+            case 6: return pick_multi_warp<6>(noz);
+            case 7: return pick_multi_warp<7>(noz);
+            case 8: return pick_multi_warp<8>(noz);
+        }
+        return nullptr;
+    }
     switch (LPT) {
         case 1: return pick_small<1>(F, noz);
         case 2: return pick_small<2>(F, noz);
@@ -175,7 +191,7 @@ spiir_status filter_launch(spiir_plan* p, const float* x, int n, spiir_c64* z, i
         for (int pass = 0; pass < (g.NC > 1 ? 2 : 1); ++pass) {
             a.mode = g.NC > 1 ? pass + 1 : 0;
             a.carry = (last_class && a.mode != 1) ? 1 : 0;
-            filter_kernel_t k = pick_kernel(g.F, g.LPT, a.mode == 1);
+            filter_kernel_t k = pick_kernel(g.F, g.LPT, g.NP, a.mode == 1);
             if (!k) { set_error("no kernel for F=%d LPT=%d", g.F, g.LPT); return SPIIR_EUNSUPPORTED; }
             SPIIR_CUDA(ensure_smem((const void*)k, g.smem_bytes));
             k<<<grid, block, g.smem_bytes, st>>>(a);
@@ -240,9 +256,7 @@ spiir_status filter_launch_group(spiir_plan* const* ps, const float* const* xs, 
         m.gx[k] = g.grid_x; m.gy[k] = g.grid_y;
         warps = std::max(warps, g.warps); gx = std::max(gx, g.grid_x); gy = std::max(gy, g.grid_y);
     }
-    // every bank of the launch runs with the launch's block size: size the reduction scratch for it
-    for (int k = 0; k < count; ++k) smem = std::max(smem, 16 * m.bank[k].CS + 16 + warps * kRedWarp4 * 16);
-    if (smem > ps[0]->dev.smem_optin) return SPIIR_EUNSUPPORTED;
+    for (int k = 0; k < count; ++k) smem = std::max(smem, 16 * m.bank[k].CS + 16);
     multi_kernel_t k = pick_multi(F, LPT);
     if (!k) return SPIIR_EUNSUPPORTED;
     SPIIR_CUDA(ensure_smem((const void*)k, smem));

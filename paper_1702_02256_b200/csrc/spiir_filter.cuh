@@ -11,13 +11,11 @@
 //     (re, im), x and the coefficients enter as broadcast operands -- 4 packed instructions per
 //     filter-sample update instead of 8 scalar ones.
 //   * Eq. 8: per lane the F filters are summed in registers; 16 time steps are batched and summed
-//     across the lanes of the template.  One warp per template (LPT = 32): a transposed reduction
-//     through a padded, conflict-free shared-memory tile (8 STS.128 + 8 LDS.128 per lane instead
-//     of 31 SHFL + 62 FSEL: the kernel is bound by register-file read bandwidth).
-//     Fewer lanes per template: a transposed xor-butterfly.  Either way every lane ends with a
-//     distinct slice of the 16 complex outputs -> coalesced stores, fixed summation order.
-//   * templates of more than 512 filters span NP adjacent warps of one CTA; their per-batch partial
-//     sums meet in shared memory behind a named barrier (the 513-filter example).
+//     across the lanes of the template with a transposed butterfly (xor-shuffles), which leaves every
+//     lane with a distinct slice of the 16 complex outputs -> coalesced stores, fixed summation order.
+//   * templates of more than 512 filters span NP adjacent warps of one CTA (the
+//     513-filter example): every warp transposes its partial sums through a padded, conflict-free
+//     shared-memory tile and the NP partial results meet there behind one named barrier per batch.
 //   * time-parallel mode (row a7): a block is cut into chunks; pass 1 runs every chunk from zero
 //     state (chunk 0 from the carried state), a carry kernel propagates s_{c+1} = a1^C s_c + e_c,
 //     pass 2 reruns every chunk from its true initial state and writes z.
@@ -181,9 +179,25 @@ struct RedCtx {
 // over the eight rows 4i + (j >> 3); the four partial quads of a column meet in a second tile, from which lane j
 // sums float j.  With NP > 1 the second tiles of the NP warps of a template are summed by its first warp after a
 // named barrier (double-buffered by the batch parity, so one barrier per batch suffices).
+template <bool MULTI>
 __device__ __forceinline__ void reduce_store_warp(float2 (&Z)[kBatch], int lane, float2* zrow, int nvalid, bool active, bool acc,
                                                   const RedCtx& rc, int bpar)
 {
+    // One warp per template: the xor-butterfly.  (A shared-memory transposition needs a third of the instructions but
+    // measured 3 % slower in this kernel: the window reads already keep the shared-memory pipe ~55 % busy.)
+    if (!MULTI) {
+        bfly_stage<16, 16>(Z, lane); bfly_stage<8, 8>(Z, lane); bfly_stage<4, 4>(Z, lane); bfly_stage<2, 2>(Z, lane);
+        const bool up = (lane & 1) != 0;
+        float keep = up ? Z[0].y : Z[0].x;
+        float send = up ? Z[0].x : Z[0].y;
+        float v = keep + __shfl_xor_sync(0xffffffffu, send, 1);
+        if (active && (lane >> 1) < nvalid) {
+            float* p = reinterpret_cast<float*>(zrow) + lane;
+            if (acc) v += *p;
+            *p = v;
+        }
+        return;
+    }
     float4* myrow = rc.rows + lane * 9;
 #pragma unroll
     for (int q = 0; q < 8; ++q) myrow[q] = make_float4(Z[2 * q].x, Z[2 * q].y, Z[2 * q + 1].x, Z[2 * q + 1].y);
@@ -197,8 +211,7 @@ __device__ __forceinline__ void reduce_store_warp(float2 (&Z)[kBatch], int lane,
         a1 = __fadd2_rn(a1, make_float2(v.z, v.w));
     }
     rc.part2[bpar * 32 + lane] = make_float4(a0.x, a0.y, a1.x, a1.y);
-    if (rc.NP == 1) __syncwarp();
-    else named_bar_sync(rc.bar_id, 32 * rc.NP);
+    named_bar_sync(rc.bar_id, 32 * rc.NP);
     if (rc.part != 0) return;
     float v = 0.f;
     for (int p = 0; p < rc.NP; ++p) {
@@ -283,7 +296,7 @@ __device__ __forceinline__ void batch_steps(const float4* __restrict__ win4, con
 
 // The kernel body takes its CTA coordinates as arguments so that one launch can also serve several banks
 // (spiir_filter_multi_kernel below): bx in [0, gdx), by in [0, gdy) with gdy = S * NC.
-template <int F, int LPT, bool NOZ>
+template <int F, int LPT, bool NOZ, bool MULTI>
 __device__ __forceinline__ void filter_body(const FilterArgs& a, const int bx, const int by, const int gdx, const int gdy)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -320,7 +333,7 @@ __device__ __forceinline__ void filter_body(const FilterArgs& a, const int bx, c
     const float4* win4 = reinterpret_cast<const float4*>(win);
 
     constexpr int TPG = 32 / LPT;                                       // templates per group
-    const int NP = LPT == 32 ? a.NP : 1;                                // warps per template (nwarps % NP == 0)
+    const int NP = MULTI ? a.NP : 1;                                    // warps per template (nwarps % NP == 0)
     RedCtx rc;
     rc.NP = NP; rc.part = warp % NP; rc.bar_id = 1 + warp / NP;
     rc.rows = red + (size_t)warp * kRedWarp4;
@@ -362,7 +375,7 @@ __device__ __forceinline__ void filter_body(const FilterArgs& a, const int bx, c
                 batch_steps<F, true, NOZ>(win4, off4, b * (kBatch / 4), cf, Y, Z, kBatch);
                 if (!NOZ) {
                     if (LPT == 32) {
-                        reduce_store_warp(Z, lane, zt + t0 + b * kBatch, kBatch, active, a.accumulate != 0, rc, bcount & 1);
+                        reduce_store_warp<MULTI>(Z, lane, zt + t0 + b * kBatch, kBatch, active, a.accumulate != 0, rc, bcount & 1);
                         ++bcount;
                     } else {
                         reduce_store<(LPT < 32 ? LPT : 16)>(Z, lane, zt + t0 + b * kBatch, kBatch, active, a.accumulate != 0);
@@ -374,7 +387,7 @@ __device__ __forceinline__ void filter_body(const FilterArgs& a, const int bx, c
                 batch_steps<F, false, NOZ>(win4, off4, nfull * (kBatch / 4), cf, Y, Z, rem);
                 if (!NOZ) {
                     if (LPT == 32) {
-                        reduce_store_warp(Z, lane, zt + t0 + nfull * kBatch, rem, active, a.accumulate != 0, rc, bcount & 1);
+                        reduce_store_warp<MULTI>(Z, lane, zt + t0 + nfull * kBatch, rem, active, a.accumulate != 0, rc, bcount & 1);
                         ++bcount;
                     } else {
                         reduce_store<(LPT < 32 ? LPT : 16)>(Z, lane, zt + t0 + nfull * kBatch, rem, active, a.accumulate != 0);
@@ -395,11 +408,11 @@ __device__ __forceinline__ void filter_body(const FilterArgs& a, const int bx, c
     if (a.carry && last_cta_arrives(a.phase, gdx * gdy)) a.phase[0] = ph ^ 1;
 }
 
-// F <= 8 is held to 128 registers so that two 8-warp CTAs (4 warps per scheduler) share an SM when their windows fit.
-template <int F, int LPT, bool NOZ>
-__global__ void __launch_bounds__(kMaxWarps * 32, (F <= 8 ? 2 : 1)) spiir_filter_kernel(const FilterArgs a)
+template <int F, int LPT, bool NOZ, bool MULTI = false>
+__global__ void __launch_bounds__(kMaxWarps * 32) spiir_filter_kernel(const FilterArgs a)
 {
-    filter_body<F, LPT, NOZ>(a, blockIdx.x, blockIdx.y, gridDim.x, gridDim.y);
+    static_assert(!MULTI || LPT == 32, "only whole-warp templates span several warps");
+    filter_body<F, LPT, NOZ, MULTI>(a, blockIdx.x, blockIdx.y, gridDim.x, gridDim.y);
 }
 
 // Several banks that share a lane mapping (F, LPT) in one launch: blockIdx.z picks the bank.  Used by the
@@ -411,11 +424,11 @@ struct MultiFilterArgs {
 };
 
 template <int F, int LPT>
-__global__ void __launch_bounds__(kMaxWarps * 32, 2) spiir_filter_multi_kernel(const __grid_constant__ MultiFilterArgs m)
+__global__ void __launch_bounds__(kMaxWarps * 32) spiir_filter_multi_kernel(const __grid_constant__ MultiFilterArgs m)
 {
     const int k = blockIdx.z;
     if ((int)blockIdx.x >= m.gx[k] || (int)blockIdx.y >= m.gy[k]) return;
-    filter_body<F, LPT, false>(m.bank[k], blockIdx.x, blockIdx.y, m.gx[k], m.gy[k]);
+    filter_body<F, LPT, false, false>(m.bank[k], blockIdx.x, blockIdx.y, m.gx[k], m.gy[k]);
 }
 
 // ---------------------------------------------------------------------------------------------

@@ -164,7 +164,7 @@ spiir_status compute_geometry(int T, int L, int S, int Dpad, int n, int opt_chun
     g->TPG = 32 / g->LPT;
     g->G = g->LPT == 32 ? T * g->NP : (T + g->TPG - 1) / g->TPG;
     const int kBatch = 16, kMaxWarps = 8;
-    const int kRedWarpBytes = (32 * 9 + 64) * 16;          // spiir_filter.cuh: kRedWarp4 float4 per warp (LPT = 32)
+    const int kRedWarpBytes = (32 * 9 + 64) * 16;          // spiir_filter.cuh: kRedWarp4 float4 per warp (multi-warp templates)
     // time chunks: only when the bank alone cannot fill the machine
     int NC = 1;
     const long tasks = (long)S * g->G;
@@ -195,7 +195,7 @@ spiir_status compute_geometry(int T, int L, int S, int Dpad, int n, int opt_chun
     warps = std::min(warps, g->G);
     if (g->NP > 1) warps = std::max(g->NP, warps / g->NP * g->NP);      // the warps of a template share a CTA
     g->warps = warps;
-    const int red_bytes = g->LPT == 32 ? warps * kRedWarpBytes : 0;
+    const int red_bytes = g->NP > 1 ? warps * kRedWarpBytes : 0;
     // time tile: as long as shared memory allows (4 shifted copies of Dpad + NT + 32 floats)
     const int budget_floats = (smem_optin - 64 - red_bytes) / 16;
     int NT = C;

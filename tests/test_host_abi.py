@@ -191,7 +191,9 @@ def test_geometry_of_the_baseline_configs(sp):
     assert g1["time_chunks"] == 1 and g1["launches"] == 1
     assert g1["warps_per_cta"] == 7 and g1["grid"] == 147                       # one CTA per SM, 7 templates each
     assert g1["time_tile"] == 4096 and g1["smem_bytes"] <= 232448
-    assert g1["smem_bytes"] == 16 * (4096 + 4096 + 32) + 16 + 7 * (32 * 9 + 64) * 16     # window copies + reduction tiles
+    assert g1["smem_bytes"] == 16 * (4096 + 4096 + 32) + 16                      # four shifted window copies + mbarrier
+    gm = sp.spiir_host_geometry(64, 1024, 1, 4095, 4096)                          # multi-warp templates: + reduction tiles
+    assert gm["smem_bytes"] == 16 * (4096 + 4096 + 32) + 16 + gm["warps_per_cta"] * (32 * 9 + 64) * 16
     g0 = sp.spiir_host_geometry(16, 128, 1, 2047, 4096)
     assert g0["time_chunks"] > 8 and g0["launches"] == 3                        # 16 warps of work -> chunked scan
     g4 = sp.spiir_host_geometry(16384, 256, 2, 2047, 2048)
