@@ -1,8 +1,8 @@
 #!/usr/bin/env python
 """bench.py -- SPIIR filter-sample updates/s on one B200 (BASELINE.json metric), with roofline,
-end-to-end and CPU-oracle legs.
+end-to-end, secondary legs and CPU-oracle legs.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1] [--impl ours|reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1] [--impl ours|reference|paper_design]
 
 A "step" is one streamed block of the workload through the whole hot path (spiir_filter, or
 spiir_mr_filter for config 3): for the default workload (BASELINE.json configs[1], the config the
@@ -18,7 +18,13 @@ Timed legs:
               block back to pinned host memory (double-buffered on a copy stream).
   roofline  : FP32 ALU bound: 12 flop per update / kernel time, against
               SMs x 128 lanes x 2 flop x clocks.max.sm (DESIGN.md derives it).
-  cpu_baseline : the float64 oracle, as it stands, on this box's host cores, on a bounded sample.
+  legs      : (default run only) the other driver-visible numbers, each timed the same way for a few
+              milliseconds: configs[4], configs[3] (roofline counts the FIR FMAs), configs[0], the
+              configs[2] sweep ends (L = 1 and 32; streamed 256-sample blocks and one bulk call of
+              16384 samples), the exported x2 stages alone (HBM and FP32 fractions), and the paper's
+              own kernel design on configs[1] (spiir_pd_filter).
+  cpu_baseline : the float64 oracle, as it stands, on this box's host cores, on a bounded sample,
+              timed in a fresh subprocess (no CUDA / NVML threads beside it): all cores and one thread.
 """
 from __future__ import annotations
 
@@ -40,14 +46,25 @@ METRIC = "SPIIR filter-sample updates/s (templates*filters*samples/s)"
 UNIT = "updates/s"
 FLOP_PER_UPDATE = 12
 FP32_LANES_PER_SM = 128         # B200 SM: 4 sub-partitions x 32 FP32 lanes (guides/B300_MICROARCH.md)
-# dram__bytes_read.sum + dram__bytes_write.sum of one spiir_filter_kernel launch, from the committed
-# `ncu --set full` captures (profiles/r1c_summary.md); per launch, like roofline.achieved
+HBM_FALLBACK_GBS = 7700.0       # B200_PROFILING.md nominal figure, used only when MEASURED_PEAKS.json is absent
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE spiir_filter_kernel launch, copied from the committed
+# `ncu --set full` captures named in TRAFFIC_SOURCE; per launch, like roofline.achieved.  Not measured by this run.
 NCU_DRAM_TRAFFIC = {"cfg1_many_filter_1024x256": 7.428352e6 + 0.137472e6,
                     "cfg4_full_bank_2x16384x256": 235.036672e6 + 556.152064e6}
+TRAFFIC_SOURCE = ("constant from the ncu --set full capture in profiles/ (r1c_summary.md), not measured by this run; "
+                  "configs[1]: coefficients, delays and state once per block; the 33.5 MB SNR block is still in the "
+                  "126 MB L2 when the kernel ends and is evicted by the flush outside the events")
 
 
 def _dist_env():
     return int(os.environ.get("RANK", "0")), int(os.environ.get("LOCAL_RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
+
+
+def load_peaks():
+    try:
+        return json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:
+        return {}
 
 
 class ClockSampler(threading.Thread):
@@ -138,17 +155,64 @@ def make_workload(cfg: int, rank: int, n_filters: int = 0):
     return w
 
 
-def make_plan(sp, w, flags=0, time_chunks=0):
+def make_plan(sp, w, flags=0, time_chunks=0, impl="ours", block=None):
+    block = block or w.block
+    if impl == "paper_design":
+        if len(w.banks) != 1 or w.n_streams != 1:
+            raise ValueError("--impl paper_design covers the single-rate, single-stream configs (0, 1, 2)")
+        b = w.banks[0]
+        plan = sp.PaperDesignPlan(b.a1, b.b0, b.delays, max_block=block)
+        return plan, 3                                  # window staging, filter kernel, history carry (+ one memset node)
     if len(w.banks) == 1:
         b = w.banks[0]
-        plan = sp.Plan(b.a1, b.b0, b.delays, b.rate_hz, n_streams=w.n_streams, max_block=w.block, flags=flags,
+        plan = sp.Plan(b.a1, b.b0, b.delays, b.rate_hz, n_streams=w.n_streams, max_block=block, flags=flags,
                        time_chunks=time_chunks)
-        launches = plan.launch_info(w.block)["launches"]
+        launches = plan.launch_info(block)["launches"]
     else:
         plan = sp.MultiratePlan([(b.a1, b.b0, b.delays) for b in w.banks], [b.rate_hz for b in w.banks],
-                                n_streams=w.n_streams, max_block=w.block)
-        launches = plan.launches(w.block)
+                                n_streams=w.n_streams, max_block=block)
+        launches = plan.launches(block)
     return plan, launches
+
+
+def fir_fma_per_block(w, n_taps_down=192, n_taps_up=192):
+    """FIR multiply-adds of one multirate block: every up-stage output is a complex sample =
+    n_taps_up/2 taps x (re, im) = n_taps_up FMAs, for every (stream, template); every down-stage output is
+    n_taps_down FMAs, once per stream."""
+    H = len(w.banks)
+    if H == 1:
+        return 0
+    up_out = sum(w.block >> h for h in range(H - 1))           # outputs per row over all up stages (4096 + ... + 128)
+    down_out = sum(w.block >> h for h in range(1, H))
+    return w.n_streams * (w.n_templates * up_out * n_taps_up + down_out * n_taps_down)
+
+
+# -------------------------------------------------------------------------------------------------
+# CPU legs (the oracle).  They run in a process that has no CUDA context, no NVML sampler and no torch
+# thread pool beside the OpenMP team: `--impl reference` is such a process itself; the GPU arm spawns one.
+# -------------------------------------------------------------------------------------------------
+def cpu_model() -> str:
+    try:
+        for ln in open("/proc/cpuinfo"):
+            if ln.lower().startswith("model name"):
+                return ln.split(":", 1)[1].strip()
+    except Exception:
+        pass
+    return "unknown"
+
+
+def usable_cores() -> int:
+    try:
+        return len(os.sched_getaffinity(0))
+    except Exception:
+        return os.cpu_count() or 1
+
+
+def oracle_env(threads: int) -> dict:
+    env = dict(os.environ)
+    env.update({"OMP_NUM_THREADS": str(threads), "OMP_PROC_BIND": "close", "OMP_PLACES": "cores", "OMP_DYNAMIC": "false",
+                "CUDA_VISIBLE_DEVICES": ""})
+    return env
 
 
 def oracle_sample(w, budget_updates: float):
@@ -158,13 +222,6 @@ def oracle_sample(w, budget_updates: float):
     T_s = int(min(w.n_templates, max(8, budget_updates // (2 * per_template_block))))
     n_b = int(max(1, min(256, budget_updates // (T_s * per_template_block))))
     return T_s, n_b
-
-
-def calibrated_oracle_sample(w, seconds: float):
-    """Pick a sample that keeps the oracle busy for about `seconds` on this box's cores."""
-    T0 = min(w.n_templates, 64)
-    rate, _, _ = run_oracle(w, T0, 1)
-    return oracle_sample(w, rate * seconds)
 
 
 def run_oracle(w, T_s: int, n_b: int):
@@ -179,6 +236,43 @@ def run_oracle(w, T_s: int, n_b: int):
     dt = time.perf_counter() - t0
     upd = w.updates_per_block() / w.n_templates * T_s * n_b
     return upd / dt, dt, oracle.num_threads()
+
+
+def calibrated_oracle_sample(w, seconds: float):
+    """Pick a sample that keeps the oracle busy for about `seconds` on this box's cores."""
+    T0 = min(w.n_templates, 64)
+    run_oracle(w, T0, 1)                                  # page the library and the inputs in
+    rate, _, _ = run_oracle(w, T0, 1)
+    return oracle_sample(w, rate * seconds)
+
+
+def cpu_leg_main(args):
+    """Child process of the GPU arm: one oracle timing with the thread count given by OMP_NUM_THREADS."""
+    w = make_workload(args.config, 0, args.filters)
+    T_s, n_b = calibrated_oracle_sample(w, args.cpu_seconds)
+    v, dt, cores = run_oracle(w, T_s, n_b)
+    print(json.dumps({"value": v, "seconds": dt, "cores": cores,
+                      "sample": f"first {T_s} of {w.n_templates} templates x {n_b} block(s) of {w.block} samples"}), flush=True)
+    return 0
+
+
+def cpu_leg_subprocess(cfg: int, filters: int, seconds: float, threads: int):
+    cmd = [sys.executable, os.path.abspath(__file__), "--cpu-leg", "--config", str(cfg), "--filters", str(filters),
+           "--cpu-seconds", str(seconds)]
+    out = subprocess.run(cmd, env=oracle_env(threads), capture_output=True, text=True, timeout=600)
+    for ln in reversed(out.stdout.strip().splitlines()):
+        if ln.startswith("{"):
+            return json.loads(ln)
+    raise RuntimeError("cpu leg failed: " + out.stderr[-400:])
+
+
+def cpu_baseline(cfg: int, filters: int, seconds: float):
+    cores = usable_cores()
+    allc = cpu_leg_subprocess(cfg, filters, seconds, cores)
+    one = cpu_leg_subprocess(cfg, filters, max(3.0, seconds / 3.0), 1)
+    return {"value": allc["value"], "unit": UNIT, "cores": allc["cores"], "kind": "oracle", "seconds": allc["seconds"],
+            "sample": allc["sample"], "single_thread": {"value": one["value"], "seconds": one["seconds"], "sample": one["sample"]},
+            "cpu_model": cpu_model(), "how": "fresh subprocess, no CUDA context, OMP_PROC_BIND=close"}
 
 
 def bench_reference(args):
@@ -200,11 +294,168 @@ def bench_reference(args):
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": float(np.mean(times) * 1e3),
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": w.name, "sample": sample},
-            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample,
+                             "cpu_model": cpu_model()},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line), flush=True)
     return 0
+
+
+# -------------------------------------------------------------------------------------------------
+# Device timing
+# -------------------------------------------------------------------------------------------------
+class DeviceTimer:
+    """K steps, each bracketed by CUDA events on the launching stream, an L2 flush (256 MiB write) between
+    steps outside the events."""
+
+    def __init__(self):
+        import torch
+        self.torch = torch
+        self.flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+        self.stream = torch.cuda.current_stream()
+
+    def run(self, step, steps: int, warmup: int, first: int = 0):
+        torch = self.torch
+        for i in range(warmup):
+            step(first + i)
+        torch.cuda.synchronize()
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+        t0 = time.perf_counter()
+        for i in range(steps):
+            self.flush.fill_(i & 0xFF)
+            ev[i][0].record(self.stream)
+            step(first + warmup + i)
+            ev[i][1].record(self.stream)
+        torch.cuda.synchronize()
+        wall = time.perf_counter() - t0
+        return np.array([a.elapsed_time(b) for a, b in ev]), wall
+
+
+def graph_steps(torch, plan, x_dev, out, mode: str):
+    """One CUDA graph per resident strain block (the library keeps every ping-pong phase on the device, so a
+    captured call can be replayed for each block of the stream); eager launches if capture fails."""
+    plan.filter(x_dev[0], out)                      # first call outside any capture (kernel attributes)
+    torch.cuda.synchronize()
+    graphs = None
+    if mode != "off":
+        try:
+            graphs = []
+            for xb in x_dev:
+                g = torch.cuda.CUDAGraph()
+                # thread_local: CUDA calls of other threads (NCCL watchdog, clock sampler) must not invalidate the capture
+                with torch.cuda.graph(g, capture_error_mode="thread_local"):
+                    plan.filter(xb, out)
+                graphs.append(g)
+        except Exception as exc:                     # pragma: no cover - depends on the driver
+            if mode == "on":
+                raise
+            print(f"bench.py: CUDA graph capture failed ({exc}); eager launches", file=sys.stderr)
+            graphs = None
+    plan.reset()
+    torch.cuda.synchronize()
+    nblk = len(x_dev)
+    if graphs is not None:
+        return (lambda i: graphs[i % nblk].replay()), True
+    return (lambda i: plan.filter(x_dev[i % nblk], out)), False
+
+
+def fp32_peak_tflops(props, sm_max_mhz):
+    return props.multi_processor_count * FP32_LANES_PER_SM * 2 * sm_max_mhz * 1e6 / 1e12
+
+
+def filter_leg(sp, timer, cfg: int, steps: int, warmup: int, peak_tflops: float, filters: int = 0, impl: str = "ours",
+               bulk_blocks: int = 0, graph: str = "auto"):
+    """One secondary leg: configs[cfg] (or its bulk shape: bulk_blocks blocks in ONE call) timed like the main leg."""
+    import torch
+    w = make_workload(cfg, 0, filters)
+    n = w.block * (bulk_blocks or 1)
+    plan, launches = make_plan(sp, w, impl=impl, block=n)
+    nblk = 2 if bulk_blocks else min(w.n_blocks, 8)
+    if bulk_blocks:
+        xs = [np.concatenate([w.strain(k * bulk_blocks + i) for i in range(bulk_blocks)], -1) for k in range(nblk)]
+    else:
+        xs = [w.strain(i) for i in range(nblk)]
+    x_dev = [torch.from_numpy(x).cuda() for x in xs]
+    out = torch.empty((w.n_streams, w.n_templates, n), dtype=torch.complex64, device="cuda")
+    step, graphed = graph_steps(torch, plan, x_dev, out, graph)
+    ms, _ = timer.run(step, steps, warmup)
+    upd = w.updates_per_block() * (bulk_blocks or 1)
+    t = float(ms.mean()) * 1e-3
+    fir = fir_fma_per_block(w)
+    flop = FLOP_PER_UPDATE * upd + 2 * fir
+    snr_bytes = w.n_streams * w.n_templates * n * 8
+    leg = {"workload": w.name + (f"_bulk{n}" if bulk_blocks else ""), "impl": impl, "ms_per_step": t * 1e3, "steps": steps,
+           "value": upd / t, "unit": UNIT, "launches_per_step": launches, "graph": graphed,
+           "roofline": {"bound": "alu", "achieved": flop / t / 1e12, "peak": peak_tflops, "unit": "TFLOP/s",
+                        "frac": flop / t / 1e12 / peak_tflops},
+           "snr_writeback_gbs": snr_bytes / t / 1e9}
+    if fir:
+        leg["roofline"]["flop"] = {"filter_updates_x12": FLOP_PER_UPDATE * upd, "fir_fma_x2": 2 * fir}
+    plan.close()
+    del plan, out, x_dev
+    torch.cuda.empty_cache()
+    return leg
+
+
+def resample_leg(sp, timer, direction: str, taps: int, rows: int, steps: int, warmup: int, hbm_peak: float, fma_peak: float):
+    """The exported x2 stage alone on a batch large enough to leave the launch-bound regime (rows x 2048 -> 4096 up with
+    accumulate, or rows x 4096 -> 2048 down).  Both rooflines DESIGN.md discusses: HBM (algorithmic bytes per output) and FP32."""
+    import torch
+    up = direction == "up"
+    n_in = 2048 if up else 4096
+    r = sp.Resampler("up" if up else "down", rows, max_block=n_in, n_taps=taps)
+    if up:
+        v = torch.randn(rows, n_in, dtype=torch.complex64, device="cuda")
+        out = torch.zeros(rows, 2 * n_in, dtype=torch.complex64, device="cuda")
+        call = lambda i: r.up(v, out, accumulate=True)
+        n_out, bytes_per_out, fma_per_out = rows * 2 * n_in, 20.0, taps            # 4 in + 8 read + 8 written; taps/2 x (re, im)
+    else:
+        u = torch.randn(rows, n_in, dtype=torch.float32, device="cuda")
+        out = torch.zeros(rows, n_in // 2, dtype=torch.float32, device="cuda")
+        call = lambda i: r.down(u, out)
+        n_out, bytes_per_out, fma_per_out = rows * n_in // 2, 12.0, taps           # 8 in + 4 written; one FMA per tap
+    ms, _ = timer.run(call, steps, max(3, warmup))
+    t = float(ms.mean()) * 1e-3
+    gbs = n_out * bytes_per_out / t / 1e9
+    leg = {"workload": f"resample_{direction}_{rows}x{n_in}_{taps}taps", "ms_per_step": t * 1e3, "steps": steps,
+           "value": n_out / t, "unit": "output samples/s",
+           "roofline": {"bound": "hbm", "achieved": gbs, "peak": hbm_peak, "unit": "GB/s", "frac": gbs / hbm_peak,
+                        "bytes_per_output": bytes_per_out},
+           "roofline_alu": {"bound": "alu", "achieved": n_out * fma_per_out * 2 / t / 1e12, "peak": 2 * fma_peak / 1e12,
+                            "unit": "TFLOP/s", "frac": n_out * fma_per_out / t / fma_peak, "fma_per_output": fma_per_out}}
+    r.close()
+    del r, out
+    torch.cuda.empty_cache()
+    return leg
+
+
+def secondary_legs(sp, timer, peak_tflops, hbm_peak, fma_peak, warmup):
+    legs = {}
+
+    def add(name, fn):
+        try:
+            legs[name] = fn()
+        except Exception as exc:                      # a failed leg must not take the headline line down with it
+            legs[name] = {"error": f"{type(exc).__name__}: {exc}"[:300]}
+
+    add("cfg4", lambda: filter_leg(sp, timer, 4, 10, 3, peak_tflops))
+    add("cfg3", lambda: filter_leg(sp, timer, 3, 50, warmup, peak_tflops))
+    add("cfg0", lambda: filter_leg(sp, timer, 0, 50, warmup, peak_tflops))
+    for L in (1, 32):
+        add(f"cfg2_L{L}_streamed", lambda L=L: filter_leg(sp, timer, 2, 100, warmup, peak_tflops, filters=L))
+        add(f"cfg2_L{L}_bulk", lambda L=L: filter_leg(sp, timer, 2, 20, 3, peak_tflops, filters=L, bulk_blocks=64))
+    add("resample_up_192", lambda: resample_leg(sp, timer, "up", 192, 16384, 20, 3, hbm_peak, fma_peak))
+    add("resample_down_192", lambda: resample_leg(sp, timer, "down", 192, 16384, 20, 3, hbm_peak, fma_peak))
+    add("resample_up_32", lambda: resample_leg(sp, timer, "up", 32, 16384, 20, 3, hbm_peak, fma_peak))
+    add("paper_design_cfg1", lambda: filter_leg(sp, timer, 1, 10, 3, peak_tflops, impl="paper_design"))
+    for L in (1, 32):
+        key = f"cfg2_L{L}_bulk"
+        if "error" not in legs.get(key, {"error": 1}):
+            # SURVEY.md H6: L <= 4 is bound by the complex64 SNR writeback (8 B per template-sample)
+            legs[key]["roofline_hbm"] = {"bound": "hbm", "achieved": legs[key]["snr_writeback_gbs"], "peak": hbm_peak,
+                                         "unit": "GB/s", "frac": legs[key]["snr_writeback_gbs"] / hbm_peak}
+    return legs
 
 
 def bench_ours(args):
@@ -220,15 +471,21 @@ def bench_ours(args):
     sp.lib()
 
     w = make_workload(args.config, rank, args.filters)
-    plan, launches = make_plan(sp, w, args.plan_flags, args.time_chunks)
-    S, T, n = w.n_streams, w.n_templates, w.block
-    upd = w.updates_per_block()
-    nblk = min(w.n_blocks, 16)
-    x_host = [torch.from_numpy(w.strain(i)).pin_memory() for i in range(nblk)]
+    bulk = args.bulk if args.config == 2 else 0
+    n = w.block * (bulk or 1)
+    plan, launches = make_plan(sp, w, args.plan_flags, args.time_chunks, impl=args.impl, block=n)
+    S, T = w.n_streams, w.n_templates
+    upd = w.updates_per_block() * (bulk or 1)
+    nblk = 2 if bulk else min(w.n_blocks, 16)
+    if bulk:
+        strains = [np.concatenate([w.strain(k * bulk + i) for i in range(bulk)], -1) for k in range(nblk)]
+    else:
+        strains = [w.strain(i) for i in range(nblk)]
+    x_host = [torch.from_numpy(x).pin_memory() for x in strains]
     x_dev = [x.cuda() for x in x_host]
     out = torch.empty((S, T, n), dtype=torch.complex64, device="cuda")
-    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
-    stream = torch.cuda.current_stream()
+    timer = DeviceTimer()
+    stream = timer.stream
 
     def barrier():
         torch.cuda.synchronize()
@@ -236,53 +493,17 @@ def bench_ours(args):
             dist.barrier()
             torch.cuda.synchronize()
 
-    # One CUDA graph per resident strain block (the library keeps every ping-pong phase on the device, so
-    # a captured call can be replayed for each block of the stream); eager launches if capture fails.
-    def capture(xbuf, obuf):
-        g = torch.cuda.CUDAGraph()
-        # thread_local: CUDA calls of other threads (NCCL watchdog, clock sampler) must not invalidate the capture
-        with torch.cuda.graph(g, capture_error_mode="thread_local"):
-            plan.filter(xbuf, obuf)
-        return g
-
-    plan.filter(x_dev[0], out)                      # first call outside any capture (kernel attributes)
-    torch.cuda.synchronize()
-    graphs = None
-    if args.graph != "off":
-        try:
-            graphs = [capture(x_dev[i], out) for i in range(nblk)]
-        except Exception as exc:                     # pragma: no cover - depends on the driver
-            if args.graph == "on":
-                raise
-            print(f"bench.py: CUDA graph capture failed ({exc}); eager launches", file=sys.stderr)
-            graphs = None
-        plan.reset()
-        torch.cuda.synchronize()
-
-    def step(i):
-        if graphs is not None:
-            graphs[i % nblk].replay()
-        else:
-            plan.filter(x_dev[i % nblk], out)
+    step, graphed = graph_steps(torch, plan, x_dev, out, args.graph)
 
     # ---- device-resident leg -------------------------------------------------------------------
     for i in range(args.warmup):
         step(i)
     barrier()
     sampler = ClockSampler(local_rank); sampler.start()
-    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
-    t_wall0 = time.perf_counter()
-    for i in range(args.steps):
-        flush.fill_(i & 0xFF)                       # L2 flush between timed steps (outside the events)
-        ev[i][0].record(stream)
-        step(args.warmup + i)
-        ev[i][1].record(stream)
+    step_ms, t_wall = timer.run(step, args.steps, 0, first=args.warmup)
     barrier()
-    t_wall = time.perf_counter() - t_wall0
     clocks = sampler.stop()
-    step_ms = np.array([a.elapsed_time(b) for a, b in ev])
-    tot_ms = float(step_ms.sum())
-    tot_ms = max_over_ranks(tot_ms, world, "cuda")
+    tot_ms = max_over_ranks(float(step_ms.sum()), world, "cuda")
     ms_per_step = tot_ms / args.steps
     value = upd * world / (ms_per_step * 1e-3)
 
@@ -295,9 +516,14 @@ def bench_ours(args):
     freed = [torch.cuda.Event() for _ in range(2)]
 
     e2e_graphs = None
-    if graphs is not None:
+    if graphed:
         try:
-            e2e_graphs = [capture(xin[b], out2[b]) for b in range(2)]
+            e2e_graphs = []
+            for b in range(2):
+                g = torch.cuda.CUDAGraph()
+                with torch.cuda.graph(g, capture_error_mode="thread_local"):
+                    plan.filter(xin[b], out2[b])
+                e2e_graphs.append(g)
         except Exception:                            # pragma: no cover
             e2e_graphs = None
 
@@ -305,7 +531,7 @@ def bench_ours(args):
         for i in range(k):
             b = i & 1
             stream.wait_event(freed[b])                               # out2[b] was drained to the host
-            xin[b].copy_(x_host[(first + i) % nblk], non_blocking=True)   # H2D of this step's input
+            xin[b].copy_(x_host[(first + i) % nblk].reshape(S, n), non_blocking=True)   # H2D of this step's input
             if e2e_graphs is not None:
                 e2e_graphs[b].replay()
             else:
@@ -313,7 +539,7 @@ def bench_ours(args):
             done[b].record(stream)
             with torch.cuda.stream(copy_stream):
                 copy_stream.wait_event(done[b])
-                z_host[b].copy_(out2[b], non_blocking=True)           # D2H of this step's result
+                z_host[b].copy_(out2[b].reshape(S, T, n), non_blocking=True)           # D2H of this step's result
                 freed[b].record(copy_stream)
 
     plan.reset()
@@ -325,47 +551,59 @@ def bench_ours(args):
     stream.wait_stream(copy_stream)
     e1.record(stream)
     barrier(); copy_stream.synchronize()
-    e2e_ms = e0.elapsed_time(e1)
-    e2e_ms = max_over_ranks(e2e_ms, world, "cuda")
+    e2e_ms = max_over_ranks(e0.elapsed_time(e1), world, "cuda")
     e2e_value = upd * world * args.steps / (e2e_ms * 1e-3)
+    del out2, z_host, xin
 
     if rank == 0:
         props = torch.cuda.get_device_properties(local_rank)
-        peaks = {}
-        try:
-            peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
-        except Exception:
-            pass
+        peaks = load_peaks()
         sm_max_mhz = float(peaks.get("sm_max_mhz") or clocks.get("sm_max_mhz") or 1965.0)
-        peak_tflops = props.multi_processor_count * FP32_LANES_PER_SM * 2 * sm_max_mhz * 1e6 / 1e12
-        achieved = FLOP_PER_UPDATE * upd / (ms_per_step * 1e-3) / 1e12
+        hbm_peak = float(peaks.get("hbm_gbs") or HBM_FALLBACK_GBS)
+        peak_tflops = fp32_peak_tflops(props, sm_max_mhz)
+        fma_peak = props.multi_processor_count * FP32_LANES_PER_SM * sm_max_mhz * 1e6       # FMA lane-ops per second
+        fir = fir_fma_per_block(w)
+        flop = FLOP_PER_UPDATE * upd + 2 * fir
+        achieved = flop / (ms_per_step * 1e-3) / 1e12
+        kernel = {"ours": "spiir_filter_kernel", "paper_design": "spiir_pd_block_kernel (the paper's own design, comparison only)"}[args.impl]
         roofline = {"bound": "alu", "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s",
-                    "frac": achieved / peak_tflops, "traffic": NCU_DRAM_TRAFFIC.get(w.name),
-                    "kernel": "spiir_filter_kernel" if len(w.banks) == 1 else "spiir_filter_kernel + resamplers (whole step)",
+                    "frac": achieved / peak_tflops, "traffic": NCU_DRAM_TRAFFIC.get(w.name) if args.impl == "ours" and not bulk else None,
+                    "traffic_note": TRAFFIC_SOURCE,
+                    "kernel": kernel if len(w.banks) == 1 else "whole multirate step: spiir_filter_kernel banks + down chain + up cascade",
                     "peak_source": f"derived: {props.multi_processor_count} SMs x {FP32_LANES_PER_SM} FP32 lanes x 2 flop x "
-                                   f"{sm_max_mhz:.0f} MHz (clocks.max.sm, MEASURED_PEAKS.json); 12 flop per update (PAPER.md:88)"}
+                                   f"{sm_max_mhz:.0f} MHz (clocks.max.sm, MEASURED_PEAKS.json); 12 flop per update (PAPER.md:88)"
+                                   + ("; FIR stages counted at 2 flop per tap-FMA" if fir else "")}
+        if fir:
+            roofline["flop"] = {"filter_updates_x12": FLOP_PER_UPDATE * upd, "fir_fma_x2": 2 * fir}
         # FMA-pipe view: an update needs 8 FP32 lane-ops (4 packed FFMA2-class instructions); the pipe peak is
-        # SMs x 128 lane-ops per clock, so pipe utilisation = updates/s * 8 / (SMs * 128 * clock)
+        # SMs x 128 lane-ops per clock, so pipe utilisation = (8 x updates + FIR FMAs) / s / (SMs * 128 * clock)
         try:
             roofline["peak_measured_ffma_loop"] = sp.spiir_probe_fp32_peak()      # TFLOP/s of a register-only FFMA loop
             roofline["frac_of_measured"] = achieved / roofline["peak_measured_ffma_loop"]
         except Exception:
             pass
-        roofline["fma_pipe_frac"] = (upd / (ms_per_step * 1e-3)) * 8.0 / (props.multi_processor_count * FP32_LANES_PER_SM * sm_max_mhz * 1e6)
+        roofline["fma_pipe_frac"] = (8.0 * upd + fir) / (ms_per_step * 1e-3) / fma_peak
         snr_bytes = S * T * n * 8
+        legs = None
+        if args.legs == "on" or (args.legs == "auto" and args.config == 1 and args.impl == "ours" and world == 1 and not bulk):
+            plan.close()
+            del out, x_dev
+            torch.cuda.empty_cache()
+            legs = secondary_legs(sp, timer, peak_tflops, hbm_peak, fma_peak, min(args.warmup, 8))
         cpu = None
         if not args.no_cpu:
-            T_s, n_b = calibrated_oracle_sample(w, args.cpu_seconds)
-            v, dt, cores = run_oracle(w, T_s, n_b)
-            cpu = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "seconds": dt,
-                   "sample": f"first {T_s} of {T} templates x {n_b} block(s) of {n} samples"}
+            try:
+                cpu = cpu_baseline(args.config, args.filters, args.cpu_seconds)
+            except Exception as exc:
+                cpu = {"error": f"{type(exc).__name__}: {exc}"[:300]}
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
                 "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
                 "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-                "config": {"workload": w.name, "templates_per_gpu": T, "filters_per_template": int(sum(b.a1.shape[1] for b in w.banks)),
+                "config": {"workload": w.name + (f"_bulk{n}" if bulk else ""), "templates_per_gpu": T,
+                           "filters_per_template": int(sum(b.a1.shape[1] for b in w.banks)),
                            "streams": S, "block_samples": n, "rate_hz": w.banks[0].rate_hz,
                            "updates_per_step_per_gpu": upd, "l2": "flushed between timed steps (256 MiB write)",
-                           "launch": "one CUDA graph replay per step" if graphs is not None else "eager launches",
+                           "launch": "one CUDA graph replay per step" if graphed else "eager launches",
                            "parallelism": f"template shards x{world}, no collective"},
                 "pct_fp32_peak": 100.0 * achieved / peak_tflops,
                 "data_seconds_per_wall_second": (n / w.banks[0].rate_hz) / (ms_per_step * 1e-3),
@@ -374,10 +612,15 @@ def bench_ours(args):
                 "wall_ms_per_step_incl_flush": t_wall * 1e3 / args.steps,
                 "clocks": clocks,
                 "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": S * n * 4, "d2h_bytes_per_step": snr_bytes,
-                        "ms_per_step": e2e_ms / args.steps},
+                        "ms_per_step": e2e_ms / args.steps,
+                        "note": "bound by the D2H copy of the SNR block over PCIe, not by the kernels"},
                 "gpu_launches": launches * args.steps,
                 "roofline": roofline,
                 "cpu_baseline": cpu}
+        if args.impl != "ours":
+            line["impl"] = args.impl
+        if legs is not None:
+            line["legs"] = legs
         print(json.dumps(line), flush=True)
     if world > 1:
         dist.barrier()
@@ -386,61 +629,26 @@ def bench_ours(args):
 
 
 def bench_resample(args):
-    """Standalone x2 stage (spiir_resample_up with accumulate / spiir_resample_down) on a batch large enough
-    to leave the launch-bound regime: rows = 16384, 2048 -> 4096 (up) or 4096 -> 2048 (down), 192 taps.
-    Reports both rooflines DESIGN.md discusses: HBM (algorithmic bytes per output) and FP32 FMA."""
+    """Standalone x2 stage: see resample_leg."""
     import torch
     import paper_1702_02256_b200 as sp
     sp.lib()
     torch.cuda.set_device(0)
-    up = args.resample == "up"
-    rows, n_in, taps = args.rows, (2048 if up else 4096), args.taps
-    r = sp.Resampler("up" if up else "down", rows, max_block=n_in, n_taps=taps)
-    if up:
-        v = torch.randn(rows, n_in, dtype=torch.complex64, device="cuda")
-        out = torch.zeros(rows, 2 * n_in, dtype=torch.complex64, device="cuda")
-        call = lambda: r.up(v, out, accumulate=True)
-        n_out, bytes_per_out, fma_per_out = rows * 2 * n_in, 20.0, taps            # 4 in + 8 read + 8 written; taps/2 x (re, im)
-    else:
-        u = torch.randn(rows, n_in, dtype=torch.float32, device="cuda")
-        out = torch.zeros(rows, n_in // 2, dtype=torch.float32, device="cuda")
-        call = lambda: r.down(u, out)
-        n_out, bytes_per_out, fma_per_out = rows * n_in // 2, 12.0, taps           # 8 in + 4 written; one FMA per tap
-    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
-    stream = torch.cuda.current_stream()
-    for _ in range(max(3, args.warmup)):
-        call()
-    torch.cuda.synchronize()
-    sampler = ClockSampler(0); sampler.start()
-    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
-    for i in range(args.steps):
-        flush.fill_(i & 0xFF)
-        ev[i][0].record(stream); call(); ev[i][1].record(stream)
-    torch.cuda.synchronize()
-    clocks = sampler.stop()
-    ms = float(np.mean([a.elapsed_time(b) for a, b in ev]))
-    peaks = {}
-    try:
-        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
-    except Exception:
-        pass
-    hbm_peak = float(peaks.get("hbm_gbs") or 6542.7)
+    peaks = load_peaks()
     props = torch.cuda.get_device_properties(0)
-    sm_max_mhz = float(peaks.get("sm_max_mhz") or clocks.get("sm_max_mhz") or 1965.0)
-    fma_peak = props.multi_processor_count * FP32_LANES_PER_SM * sm_max_mhz * 1e6           # FMA lane-ops per second
-    gbs = n_out * bytes_per_out / (ms * 1e-3) / 1e9
-    line = {"metric": f"x2 resampler ({args.resample}) output samples/s", "value": n_out / (ms * 1e-3), "unit": "samples/s",
-            "n_gpus": 1, "steps": args.steps, "warmup": max(3, args.warmup), "ms_per_step": ms, "higher_is_better": True,
-            "dtype": "f32", "data": "synthetic",
-            "config": {"workload": f"resample_{args.resample}_{rows}x{n_in}_{taps}taps", "rows": rows, "n_in": n_in, "n_taps": taps,
+    timer = DeviceTimer()
+    sampler = ClockSampler(0); sampler.start()
+    sm_max_mhz = float(peaks.get("sm_max_mhz") or 1965.0)
+    fma_peak = props.multi_processor_count * FP32_LANES_PER_SM * sm_max_mhz * 1e6
+    leg = resample_leg(sp, timer, args.resample, args.taps, args.rows, args.steps, args.warmup,
+                       float(peaks.get("hbm_gbs") or HBM_FALLBACK_GBS), fma_peak)
+    clocks = sampler.stop()
+    line = {"metric": f"x2 resampler ({args.resample}) output samples/s", "value": leg["value"], "unit": "samples/s",
+            "n_gpus": 1, "steps": args.steps, "warmup": max(3, args.warmup), "ms_per_step": leg["ms_per_step"],
+            "higher_is_better": True, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": leg["workload"], "rows": args.rows, "n_taps": args.taps,
                        "l2": "flushed between timed steps (256 MiB write)"},
-            "clocks": clocks, "gpu_launches": args.steps,
-            "roofline": {"bound": "alu", "achieved": n_out * fma_per_out * 2 / (ms * 1e-3) / 1e12, "peak": 2 * fma_peak / 1e12,
-                         "unit": "TFLOP/s", "frac": n_out * fma_per_out / (ms * 1e-3) / fma_peak, "traffic": None,
-                         "kernel": f"spiir_up2_fir_kernel<{taps // 2}>" if up else f"spiir_down2_fir_kernel<{taps}>",
-                         "note": f"{taps} FMA per output sample (DESIGN.md 5.2: 192 taps are FP32-bound, 32 taps HBM-bound)"},
-            "roofline_hbm": {"bound": "hbm", "achieved": gbs, "peak": hbm_peak, "unit": "GB/s", "frac": gbs / hbm_peak,
-                             "bytes_per_output": bytes_per_out}}
+            "clocks": clocks, "gpu_launches": args.steps, "roofline": leg["roofline_alu"], "roofline_hbm": leg["roofline"]}
     print(json.dumps(line), flush=True)
     return 0
 
@@ -451,21 +659,29 @@ def main():
     ap.add_argument("--steps", type=int, default=200)
     ap.add_argument("--warmup", type=int, default=16)
     ap.add_argument("--config", type=int, default=1, help="BASELINE.json configs index (default 1: the metric's config)")
-    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference", "paper_design"],
+                    help="reference: the float64 oracle on the host cores; paper_design: the paper's own (Maxwell) kernel "
+                         "design restated for this GPU (spiir_pd_filter, comparison only)")
     ap.add_argument("--cpu-seconds", type=float, default=12.0, help="target CPU time of one oracle sample")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--legs", default="auto", choices=["auto", "on", "off"],
+                    help="secondary legs in the JSON line (auto: only in the default configs[1] run on one GPU)")
     ap.add_argument("--time-chunks", type=int, default=0, help="spiir_plan_opts.time_chunks (0 auto, 1 never chunk)")
     ap.add_argument("--filters", type=int, default=0, help="config 2 only: filters per template of the sweep point")
+    ap.add_argument("--bulk", type=int, default=0, help="config 2 only: this many 256-sample blocks in ONE call (64: n = 16384)")
     ap.add_argument("--resample", default="", choices=["", "up", "down"],
                     help="time the exported x2 stage alone (rows x 2048 -> 4096 up+accumulate, or rows x 4096 -> 2048 down)")
     ap.add_argument("--rows", type=int, default=16384, help="rows of the --resample batch")
-    ap.add_argument("--taps", type=int, default=192, choices=[32, 192],
-                    help="FIR length of the --resample stage (192: configs[3]; 32: the paper's own up-filter, PAPER.md:88)")
+    ap.add_argument("--taps", type=int, default=192, choices=[32, 192, 384],
+                    help="FIR length of the --resample stage (192: configs[3]; 32 / 384: the paper's own up / down filters, PAPER.md:88)")
     ap.add_argument("--graph", default="auto", choices=["auto", "on", "off"],
                     help="replay one captured CUDA graph per step (auto: fall back to eager launches if capture fails)")
     ap.add_argument("--plan-flags", type=int, default=0, help="spiir_plan_opts.flags (bit 0: skip the bank-conflict-avoiding permutation)")
+    ap.add_argument("--cpu-leg", action="store_true", help=argparse.SUPPRESS)
     args = ap.parse_args()
-    if args.warmup < 3 and args.impl == "ours":
+    if args.cpu_leg:
+        return cpu_leg_main(args)
+    if args.warmup < 3 and args.impl != "reference":
         args.warmup = 3
     if args.resample:
         return bench_resample(args)
@@ -475,4 +691,10 @@ def main():
 
 
 if __name__ == "__main__":
+    if "--impl" in sys.argv and "reference" in sys.argv or "--cpu-leg" in sys.argv:
+        # the oracle's OpenMP team: pinned, one thread per usable core, set before the library loads
+        os.environ.setdefault("OMP_NUM_THREADS", str(usable_cores()))
+        os.environ.setdefault("OMP_PROC_BIND", "close")
+        os.environ.setdefault("OMP_PLACES", "cores")
+        os.environ.setdefault("OMP_DYNAMIC", "false")
     sys.exit(main())
