@@ -35,7 +35,33 @@ def needs_build() -> bool:
     return any(os.path.getmtime(d) > t for d in deps)
 
 
+def _includes(path: str, seen=None) -> set:
+    """Quoted includes of a source, followed recursively (paths relative to the including file)."""
+    seen = set() if seen is None else seen
+    try:
+        text = open(path).read()
+    except OSError:
+        return seen
+    for ln in text.splitlines():
+        ln = ln.strip()
+        if ln.startswith("#include \""):
+            inc = os.path.normpath(os.path.join(os.path.dirname(path), ln.split('"')[1]))
+            if inc not in seen:
+                seen.add(inc)
+                _includes(inc, seen)
+    return seen
+
+
+def _stale(obj: str, src: str) -> bool:
+    if not os.path.exists(obj):
+        return True
+    t = os.path.getmtime(obj)
+    deps = [src, os.path.abspath(__file__)] + sorted(_includes(src))
+    return any(os.path.exists(d) and os.path.getmtime(d) > t for d in deps)
+
+
 def build(force: bool = False, verbose: bool = False) -> str:
+    """Compile every stale translation unit (in parallel) and link libspiir.so."""
     if not force and not needs_build():
         return LIB
     nvcc = _nvcc()
@@ -43,10 +69,13 @@ def build(force: bool = False, verbose: bool = False) -> str:
     objs = []
     procs = []
     for s in SOURCES:
+        src = os.path.join(CSRC, s)
         obj = os.path.join(CSRC, os.path.splitext(s)[0] + ".o")
-        cmd = [nvcc] + flags + (["-Xptxas", "-v"] if verbose else []) + ["-x", "cu", "-c", os.path.join(CSRC, s), "-o", obj]
-        procs.append((cmd, subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)))
         objs.append(obj)
+        if not force and not _stale(obj, src):
+            continue
+        cmd = [nvcc] + flags + (["-Xptxas", "-v"] if verbose else []) + ["-x", "cu", "-c", src, "-o", obj]
+        procs.append((cmd, subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)))
     for cmd, pr in procs:
         out, _ = pr.communicate()
         if verbose or pr.returncode != 0:

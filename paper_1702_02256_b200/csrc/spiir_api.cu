@@ -155,6 +155,29 @@ static filter_kernel_t pick_kernel(int F, int LPT, int NP, bool noz)
     return nullptr;
 }
 
+template <int LPT>
+static filter_kernel_t pick_scan_f(int F)
+{
+    switch (F) {
+        case 1: return (filter_kernel_t)spiir_filter_scan_kernel<1, LPT>;
+        case 2: return (filter_kernel_t)spiir_filter_scan_kernel<2, LPT>;
+        case 3: return (filter_kernel_t)spiir_filter_scan_kernel<3, LPT>;
+        case 4: return (filter_kernel_t)spiir_filter_scan_kernel<4, LPT>;
+    }
+    return nullptr;
+}
+
+static filter_kernel_t pick_scan_kernel(int F, int LPT)
+{
+    switch (LPT) {
+        case 1: return pick_scan_f<1>(F);
+        case 2: return pick_scan_f<2>(F);
+        case 4: return pick_scan_f<4>(F);
+        case 8: return pick_scan_f<8>(F);
+    }
+    return nullptr;
+}
+
 spiir_status plan_geometry(const spiir_plan* p, const spiir_bank_class& c, int n, FilterGeometry* g)
 {
     return compute_geometry(c.T, c.L, p->S, p->Dpad, n, p->opt_chunks, c.NC_cap, p->dev.n_sm, p->dev.smem_optin, g);
@@ -171,6 +194,7 @@ static void fill_filter_args(const spiir_plan* p, const spiir_bank_class& c, con
     a->NT = g.NT; a->CS = g.CS; a->NC = g.NC; a->C = g.C;
     a->x_aligned = ((reinterpret_cast<uintptr_t>(x) & 15u) == 0 && (p->S == 1 || (n & 3) == 0)) ? 1 : 0;
     a->accumulate = accumulate;
+    a->z16 = ((reinterpret_cast<uintptr_t>(z) & 15u) == 0 && (n & 1) == 0) ? 1 : 0;
     a->mode = 0;
     a->tmap = c.d_tmap; a->T_rows = p->T; a->NP = c.NP; a->carry = 0;
 }
@@ -188,6 +212,15 @@ spiir_status filter_launch(spiir_plan* p, const float* x, int n, spiir_c64* z, i
         FilterArgs a;
         fill_filter_args(p, c, x, n, z, accumulate, g, &a);
         const dim3 grid(g.grid_x, g.grid_y), block(g.warps * 32);
+        if (g.scan) {                                     // time-parallel scan inside one CTA per warp task: one launch
+            a.carry = last_class ? 1 : 0;
+            filter_kernel_t k = pick_scan_kernel(g.F, g.LPT);
+            if (!k) { set_error("no scan kernel for F=%d LPT=%d", g.F, g.LPT); return SPIIR_EUNSUPPORTED; }
+            SPIIR_CUDA(ensure_smem((const void*)k, g.smem_bytes));
+            k<<<grid, block, g.smem_bytes, st>>>(a);
+            SPIIR_CUDA(cudaGetLastError());
+            continue;
+        }
         for (int pass = 0; pass < (g.NC > 1 ? 2 : 1); ++pass) {
             a.mode = g.NC > 1 ? pass + 1 : 0;
             a.carry = (last_class && a.mode != 1) ? 1 : 0;
@@ -341,7 +374,7 @@ static spiir_status describe_classes(spiir_plan* p, const int32_t* offsets, int 
         FilterGeometry g;
         spiir_status rc = plan_geometry(p, c, p->max_block, &g);
         if (rc != SPIIR_OK) return rc;
-        int nc = g.NC;
+        int nc = g.scan ? 1 : g.NC;                       // the in-CTA scan keeps its chunk states in shared memory
         while (nc > 1 && (size_t)nc * p->S * c.nfilt * sizeof(float2) > ((size_t)256 << 20)) nc /= 2;
         c.NC_cap = std::max(1, nc);
     }

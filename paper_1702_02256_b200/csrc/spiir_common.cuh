@@ -23,4 +23,21 @@ __device__ __forceinline__ bool last_cta_arrives(int* w, int total_ctas)
     return last;                                     // meaningful in thread 0 only
 }
 
+
+// The same without any wait (filter kernels): w[1] counts kPhaseUnit per finished launch -- every CTA of a launch adds its
+// share with a fire-and-forget reduction, in any order and at any time after it has read the word -- and the phase is the
+// parity of the number of finished launches, w[1] / kPhaseUnit.  A CTA that reads the word while its own launch is
+// under way sees a partial sum below the next multiple, i.e. still the phase the launch started with.  The shares of one
+// launch add up to kPhaseUnit whatever its grid, so calls with different block lengths can follow one another.
+constexpr int kPhaseUnit = 1 << 16;                 // grids of up to 65536 CTAs; 2^32 is a multiple, so wrap-around is harmless
+__device__ __forceinline__ int phase_parity(const int* w)
+{
+    return (int)((*reinterpret_cast<const volatile unsigned*>(w + 1) >> 16) & 1u);
+}
+__device__ __forceinline__ void phase_arrive(int* w, int cta, int total_ctas)      // call from ONE thread per CTA
+{
+    const int share = kPhaseUnit / total_ctas + (cta == 0 ? kPhaseUnit % total_ctas : 0);
+    atomicAdd(reinterpret_cast<unsigned*>(w + 1), (unsigned)share);                 // result unused: compiles to RED
+}
+
 }  // namespace spiir

@@ -56,6 +56,7 @@ struct FilterArgs {
     int T_rows;              // rows of z per stream (= T unless the bank is one class of a ragged plan)
     int NP;                  // warps per template (LPT = 32 only; G = T * NP pieces)
     int carry;               // this launch writes the next input history and flips the phase
+    int z16;                 // every row of z starts 16-byte aligned (z pointer and n even): few-filter mappings store full lines
 };
 
 // shared-memory scratch of one warp for the transposed reduction (LPT = 32), in float4 units:
@@ -247,6 +248,79 @@ __device__ __forceinline__ void reduce_store(float2 (&Z)[kBatch], int lane, floa
     }
 }
 
+// Few lanes per template (LPT <= 4): after the butterfly a lane holds 16/LPT consecutive outputs of ITS template, so a
+// direct store makes every lane of a warp instruction hit a different 128-byte line with 8..32 bytes (row a5 is the bound
+// of this regime: 512 sector writes per batch).  Instead the warp's [32/LPT templates][16 steps] tile goes
+// through shared memory (rows padded to 144 bytes: conflict-free both ways) and is written as whole 128-byte lines,
+// eight lanes per row.  trow[i]: output row of tile row 4i + lane/8, or -1.
+constexpr int kTileRow4 = 9;                                   // float4 per tile row (8 + 1 padding)
+template <int LPT>
+__device__ __forceinline__ void reduce_store_tile(float2 (&Z)[kBatch], int lane, float4* tile, float2* z_s, size_t n, int tpos,
+                                                  const int (&trow)[(32 / LPT + 3) / 4], int nvalid, bool acc)
+{
+    static_assert(LPT <= 4, "wider mappings already store contiguous 16-byte pieces");
+    if (LPT >= 2) bfly_stage<16, LPT / 2>(Z, lane);
+    if (LPT >= 4) bfly_stage<8, LPT / 4>(Z, lane);
+    constexpr int NV = kBatch / LPT;                           // complex values per lane
+    float4* my = tile + (lane / LPT) * kTileRow4 + (lane % LPT) * (NV / 2);
+#pragma unroll
+    for (int i = 0; i < NV / 2; ++i) my[i] = make_float4(Z[2 * i].x, Z[2 * i].y, Z[2 * i + 1].x, Z[2 * i + 1].y);
+    __syncwarp();
+    const int q = lane & 7;
+#pragma unroll
+    for (int i = 0; i < (32 / LPT + 3) / 4; ++i) {
+        if (trow[i] >= 0 && 2 * q < nvalid) {
+            float4 v = tile[(4 * i + (lane >> 3)) * kTileRow4 + q];
+            float2* dst = z_s + (size_t)trow[i] * n + tpos + 2 * q;
+            if (2 * q + 1 < nvalid) {
+                if (acc) { const float4 o = *reinterpret_cast<const float4*>(dst); v.x += o.x; v.y += o.y; v.z += o.z; v.w += o.w; }
+                *reinterpret_cast<float4*>(dst) = v;
+            } else {
+                if (acc) { v.x += dst->x; v.y += dst->y; }
+                *dst = make_float2(v.x, v.y);
+            }
+        }
+    }
+    __syncwarp();
+}
+
+// Where a batch of 16 outputs goes: one entry point for the three reductions above.
+template <int LPT>
+struct OutCtx {
+    static constexpr int NI = LPT <= 4 ? (32 / LPT + 3) / 4 : 1;
+    float2* zt;          // this lane's template row at the block start (valid when active)
+    float2* z_s;         // row 0 of this stream
+    size_t n;
+    float4* tile;        // LPT <= 4: this warp's [32/LPT][kTileRow4] tile
+    int trow[NI];        // LPT <= 4: output row of tile row 4i + lane/8, or -1
+    bool active, acc, z16;
+};
+
+template <int LPT>
+__device__ __forceinline__ void out_ctx_rows(OutCtx<LPT>& o, const FilterArgs& a, int g, int lane)
+{
+    constexpr int TPG = 32 / LPT;
+#pragma unroll
+    for (int i = 0; i < OutCtx<LPT>::NI; ++i) {
+        const int r = 4 * i + (lane >> 3), tl = g * TPG + r;
+        o.trow[i] = (LPT <= 4 && r < TPG && tl < a.T) ? (a.tmap ? a.tmap[tl] : tl) : -1;
+    }
+}
+
+template <int LPT, bool MULTI>
+__device__ __forceinline__ void emit_batch(float2 (&Z)[kBatch], int lane, int tpos, int nvalid, const OutCtx<LPT>& o,
+                                           const RedCtx& rc, int bpar)
+{
+    if constexpr (LPT == 32) {
+        reduce_store_warp<MULTI>(Z, lane, o.zt + tpos, nvalid, o.active, o.acc, rc, bpar);
+    } else if constexpr (LPT <= 4) {
+        if (o.z16) reduce_store_tile<LPT>(Z, lane, o.tile, o.z_s, o.n, tpos, o.trow, nvalid, o.acc);
+        else reduce_store<LPT>(Z, lane, o.zt + tpos, nvalid, o.active, o.acc);
+    } else {
+        reduce_store<LPT>(Z, lane, o.zt + tpos, nvalid, o.active, o.acc);
+    }
+}
+
 // ---------------------------------------------------------------------------------------------
 // 16 time steps of Eq. 7 for the F filters of a lane.  off4[f]: float4 index of W[Dpad + j - d_f]
 // in the right shifted copy at batch start j.
@@ -302,30 +376,19 @@ __device__ __forceinline__ void filter_body(const FilterArgs& a, const int bx, c
     extern __shared__ __align__(16) unsigned char smem_raw[];
     float* win = reinterpret_cast<float*>(smem_raw);                   // 4 copies x CS floats
     uint64_t* bar = reinterpret_cast<uint64_t*>(win + 4 * (size_t)a.CS);
-    float4* red = reinterpret_cast<float4*>(win + 4 * (size_t)a.CS + 4);    // LPT = 32: kRedWarp4 float4 per warp
+    float4* red = reinterpret_cast<float4*>(win + 4 * (size_t)a.CS + 4);    // multi-warp templates: kRedWarp4 float4 per warp; LPT <= 4: store tiles
 
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
     const int s = by / a.NC, c = by % a.NC;
     const int tc0 = c * a.C;                                            // chunk range [tc0, tc1)
     const int tc1 = min(a.n, tc0 + a.C);
-    const int ph = phase_read(a.phase);
+    const int ph = phase_parity(a.phase);
+    if (a.carry && threadIdx.x == 0) phase_arrive(a.phase, by * gdx + bx, gdx * gdy);   // no one waits for this
     const float* hist_s = a.hbuf[ph] + (size_t)s * a.Dpad;
     const float* x_s = a.x + (size_t)s * a.n;
     uint32_t parity = 0;
     if (threadIdx.x == 0) mbar_init(bar, 1);
     __syncthreads();
-
-    // carried history for the next block (reads only hist + x: no race with other CTAs).  Every CTA of the
-    // stream copies a slice: one CTA doing all Dpad samples is a chain of ~Dpad/blockDim dependent global
-    // round trips (11 us for 4096 samples) that the whole launch then waits for.
-    if (a.carry) {
-        float* hn = a.hbuf[ph ^ 1] + (size_t)s * a.Dpad;
-        const int cta = c * gdx + bx, nctas = a.NC * gdx;
-        for (int i = cta * blockDim.x + threadIdx.x; i < a.Dpad; i += nctas * blockDim.x) {
-            int g = a.n - a.Dpad + i;
-            hn[i] = (g >= 0) ? x_s[g] : hist_s[a.n + i];
-        }
-    }
     const int ntiles = (tc1 - tc0 + a.NT - 1) / a.NT;
     // single-tile case: the window is staged once, AFTER the first group's coefficient / state loads have been
     // issued (below), so that their DRAM round trip overlaps the TMA copy and the shifted copies
@@ -362,7 +425,12 @@ __device__ __forceinline__ void filter_body(const FilterArgs& a, const int bx, c
             }
             Y[f] = y0;
         }
-        float2* zt = active ? a.z + ((size_t)s * a.T_rows + t) * (size_t)a.n : nullptr;
+        OutCtx<LPT> oc;
+        oc.zt = active ? a.z + ((size_t)s * a.T_rows + t) * (size_t)a.n : nullptr;
+        oc.z_s = a.z + (size_t)s * a.T_rows * (size_t)a.n; oc.n = (size_t)a.n;
+        oc.tile = red + (size_t)warp * (TPG * kTileRow4);
+        oc.active = active; oc.acc = a.accumulate != 0; oc.z16 = a.z16 != 0;
+        out_ctx_rows<LPT>(oc, a, g, lane);
         if (!staged) { stage_window(win, bar, parity, a, hist_s, x_s, tc0); staged = true; }
 
         for (int tile = 0; tile < ntiles; ++tile) {
@@ -373,26 +441,12 @@ __device__ __forceinline__ void filter_body(const FilterArgs& a, const int bx, c
             float2 Z[kBatch];
             for (int b = 0; b < nfull; ++b) {
                 batch_steps<F, true, NOZ>(win4, off4, b * (kBatch / 4), cf, Y, Z, kBatch);
-                if (!NOZ) {
-                    if (LPT == 32) {
-                        reduce_store_warp<MULTI>(Z, lane, zt + t0 + b * kBatch, kBatch, active, a.accumulate != 0, rc, bcount & 1);
-                        ++bcount;
-                    } else {
-                        reduce_store<(LPT < 32 ? LPT : 16)>(Z, lane, zt + t0 + b * kBatch, kBatch, active, a.accumulate != 0);
-                    }
-                }
+                if (!NOZ) { emit_batch<LPT, MULTI>(Z, lane, t0 + b * kBatch, kBatch, oc, rc, bcount & 1); ++bcount; }
             }
             const int rem = len - nfull * kBatch;
             if (rem > 0) {
                 batch_steps<F, false, NOZ>(win4, off4, nfull * (kBatch / 4), cf, Y, Z, rem);
-                if (!NOZ) {
-                    if (LPT == 32) {
-                        reduce_store_warp<MULTI>(Z, lane, zt + t0 + nfull * kBatch, rem, active, a.accumulate != 0, rc, bcount & 1);
-                        ++bcount;
-                    } else {
-                        reduce_store<(LPT < 32 ? LPT : 16)>(Z, lane, zt + t0 + nfull * kBatch, rem, active, a.accumulate != 0);
-                    }
-                }
+                if (!NOZ) { emit_batch<LPT, MULTI>(Z, lane, t0 + nfull * kBatch, rem, oc, rc, bcount & 1); ++bcount; }
             }
         }
         if (wactive) {
@@ -405,7 +459,21 @@ __device__ __forceinline__ void filter_body(const FilterArgs& a, const int bx, c
             }
         }
     }
-    if (a.carry && last_cta_arrives(a.phase, gdx * gdy)) a.phase[0] = ph ^ 1;
+    // carried history for the next block (reads only hist + x, writes the other buffer: no race with other CTAs).  Every
+    // CTA of the stream copies a slice, at the END of its life: by then x and the history are in L2 and the copy is off
+    // the critical path (at the top it was a chain of DRAM round trips in front of the coefficient loads).
+    if (a.carry) {
+        float* hn = a.hbuf[ph ^ 1] + (size_t)s * a.Dpad;
+        const int cta = c * gdx + bx, nctas = a.NC * gdx;
+        if (a.NC == 1 && ntiles == 1 && staged) {      // the window still holds the whole block: W[n + i] is sample n - Dpad + i
+            for (int i = cta * blockDim.x + threadIdx.x; i < a.Dpad; i += nctas * blockDim.x) hn[i] = win[a.n + i];
+        } else {
+            for (int i = cta * blockDim.x + threadIdx.x; i < a.Dpad; i += nctas * blockDim.x) {
+                int g = a.n - a.Dpad + i;
+                hn[i] = (g >= 0) ? x_s[g] : hist_s[a.n + i];
+            }
+        }
+    }
 }
 
 template <int F, int LPT, bool NOZ, bool MULTI = false>
@@ -413,6 +481,152 @@ __global__ void __launch_bounds__(kMaxWarps * 32) spiir_filter_kernel(const Filt
 {
     static_assert(!MULTI || LPT == 32, "only whole-warp templates span several warps");
     filter_body<F, LPT, NOZ, MULTI>(a, blockIdx.x, blockIdx.y, gridDim.x, gridDim.y);
+}
+
+// ---------------------------------------------------------------------------------------------
+// Time-parallel scan INSIDE one CTA (row a7 for banks that cannot fill the machine and whose blocks are
+// too short to pay for three launches: the few-filter regime, and the high-rate banks of
+// the multirate plan).  One CTA = one warp task (group g, stream s); its NCW warps split the time tile into
+// chunks of C samples.  Pass 1: warp 0 runs chunk 0 from the true state and writes z at once, warps
+// 1..nch-2 run their chunks from zero state without z; the end states meet in shared memory, every warp
+// folds s_{c+1} = a1^C s_c + e_c up to its own chunk (a1^C by repeated squaring in double), and pass 2
+// reruns chunks 1..nch-1 from their true initial states with z.  Critical path: two chunks instead of
+// the whole tile; one launch.
+// ---------------------------------------------------------------------------------------------
+constexpr int kScanMaxWarps = 16;
+
+// one chunk [cbeg, cbeg + clen) of the staged tile that starts at block sample t0
+template <int F, int LPT, bool NOZ>
+__device__ __forceinline__ void scan_run_chunk(const float4* __restrict__ win4, const int (&off4)[F], const float4 (&cf)[F],
+                                               float2 (&Y)[F], int t0, int cbeg, int clen, int lane, const OutCtx<LPT>& oc)
+{
+    const int nfull = clen / kBatch;
+    const RedCtx rc{};
+    float2 Z[kBatch];
+    for (int b = 0; b < nfull; ++b) {
+        batch_steps<F, true, NOZ>(win4, off4, (cbeg >> 2) + b * (kBatch / 4), cf, Y, Z, kBatch);
+        if (!NOZ) emit_batch<LPT, false>(Z, lane, t0 + cbeg + b * kBatch, kBatch, oc, rc, 0);
+    }
+    const int rem = clen - nfull * kBatch;
+    if (rem > 0) {
+        batch_steps<F, false, NOZ>(win4, off4, (cbeg >> 2) + nfull * (kBatch / 4), cf, Y, Z, rem);
+        if (!NOZ) emit_batch<LPT, false>(Z, lane, t0 + cbeg + nfull * kBatch, rem, oc, rc, 0);
+    }
+}
+
+template <int F, int LPT>
+__global__ void __launch_bounds__(kScanMaxWarps * 32) spiir_filter_scan_kernel(const FilterArgs a)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    float* win = reinterpret_cast<float*>(smem_raw);                   // 4 copies x CS floats
+    uint64_t* bar = reinterpret_cast<uint64_t*>(win + 4 * (size_t)a.CS);
+    float2* ex = reinterpret_cast<float2*>(win + 4 * (size_t)a.CS + 4);     // [NCW + 1][F][32]: ex[0] = state at the tile start
+
+    const int lane = threadIdx.x & 31, c = threadIdx.x >> 5, NCW = blockDim.x >> 5;
+    const int g = blockIdx.x, s = blockIdx.y;
+    constexpr int TPG = 32 / LPT;
+    const int tl = g * TPG + lane / LPT;
+    const bool active = tl < a.T;
+    const int t = active ? (a.tmap ? a.tmap[tl] : tl) : 0;
+    OutCtx<LPT> oc;
+    oc.zt = a.z + ((size_t)s * a.T_rows + t) * (size_t)a.n;
+    oc.z_s = a.z + (size_t)s * a.T_rows * (size_t)a.n; oc.n = (size_t)a.n;
+    oc.tile = reinterpret_cast<float4*>(ex + (size_t)(NCW + 1) * F * 32) + (size_t)c * (TPG * kTileRow4);
+    oc.active = active; oc.acc = a.accumulate != 0; oc.z16 = a.z16 != 0;
+    out_ctx_rows<LPT>(oc, a, g, lane);
+    const size_t lbase = ((size_t)g * F) * 32 + lane;
+    float2* st = a.state + (size_t)s * a.sstride + lbase;
+
+    // coefficient / delay / state loads first: their DRAM round trip overlaps the one of the phase word and the window
+    float4 cf[F]; float2 Y[F], aC[F]; int off4[F], dl[F];
+#pragma unroll
+    for (int f = 0; f < F; ++f) {
+        cf[f] = a.coef[lbase + (size_t)f * 32];
+        dl[f] = a.dly[lbase + (size_t)f * 32];
+        Y[f] = (c == 0) ? st[(size_t)f * 32] : make_float2(0.f, 0.f);
+    }
+    const int ph = phase_parity(a.phase);
+    if (a.carry && threadIdx.x == 0) phase_arrive(a.phase, blockIdx.y * gridDim.x + blockIdx.x, gridDim.x * gridDim.y);
+    const float* hist_s = a.hbuf[ph] + (size_t)s * a.Dpad;
+    const float* x_s = a.x + (size_t)s * a.n;
+    uint32_t parity = 0;
+    if (threadIdx.x == 0) mbar_init(bar, 1);
+    __syncthreads();
+#pragma unroll
+    for (int f = 0; f < F; ++f) {
+        const int d = dl[f];
+        const int sh = (-d) & 3;
+        off4[f] = (sh * a.CS + a.Dpad - d - sh) >> 2;
+        // a1^C, C = chunk length, by repeated squaring in double
+        double pr = 1.0, pi = 0.0, br = (double)cf[f].x, bi = (double)cf[f].y;
+        for (int e = a.C; e > 0; e >>= 1) {
+            if (e & 1) { const double r = pr * br - pi * bi, q = pr * bi + pi * br; pr = r; pi = q; }
+            const double r = br * br - bi * bi, q = 2.0 * br * bi; br = r; bi = q;
+        }
+        aC[f] = make_float2((float)pr, (float)pi);
+    }
+    const float4* win4 = reinterpret_cast<const float4*>(win);
+    const int ntiles = (a.n + a.NT - 1) / a.NT;
+    for (int tile = 0; tile < ntiles; ++tile) {
+        const int t0 = tile * a.NT;
+        const int len = min(a.NT, a.n - t0);
+        __syncthreads();                                               // window and ex[] of the previous tile are free
+        stage_window(win, bar, parity, a, hist_s, x_s, t0);
+        if (a.carry && ntiles == 1) {
+            // carried history for the next block straight from the staged window: W[n + i] is sample n - Dpad + i
+            float* hn = a.hbuf[ph ^ 1] + (size_t)s * a.Dpad;
+            for (int i = g * blockDim.x + threadIdx.x; i < a.Dpad; i += gridDim.x * blockDim.x) hn[i] = win[a.n + i];
+        }
+        const int nch = (len + a.C - 1) / a.C;
+        const int cbeg = c * a.C, clen = min(a.C, len - cbeg);
+        if (c == 0) {
+            if (tile > 0) {
+#pragma unroll
+                for (int f = 0; f < F; ++f) Y[f] = ex[f * 32 + lane];
+            }
+            scan_run_chunk<F, LPT, false>(win4, off4, cf, Y, t0, 0, clen, lane, oc);
+#pragma unroll
+            for (int f = 0; f < F; ++f) ex[((nch > 1 ? 1 : 0) * F + f) * 32 + lane] = Y[f];
+        } else if (c < nch - 1) {
+#pragma unroll
+            for (int f = 0; f < F; ++f) Y[f] = make_float2(0.f, 0.f);
+            scan_run_chunk<F, LPT, true>(win4, off4, cf, Y, t0, cbeg, clen, lane, oc);
+#pragma unroll
+            for (int f = 0; f < F; ++f) ex[((c + 1) * F + f) * 32 + lane] = Y[f];
+        }
+        __syncthreads();
+        if (c >= 1 && c < nch) {
+#pragma unroll
+            for (int f = 0; f < F; ++f) {
+                float2 v = ex[(F + f) * 32 + lane];                    // true end of chunk 0 = initial state of chunk 1
+                for (int j = 1; j < c; ++j) {
+                    const float2 e = ex[((j + 1) * F + f) * 32 + lane];
+                    float2 nx;
+                    nx.x = fmaf(aC[f].x, v.x, fmaf(-aC[f].y, v.y, e.x));
+                    nx.y = fmaf(aC[f].x, v.y, fmaf(aC[f].y, v.x, e.y));
+                    v = nx;
+                }
+                Y[f] = v;
+            }
+            scan_run_chunk<F, LPT, false>(win4, off4, cf, Y, t0, cbeg, clen, lane, oc);
+            if (c == nch - 1) {
+#pragma unroll
+                for (int f = 0; f < F; ++f) ex[f * 32 + lane] = Y[f];
+            }
+        }
+    }
+    __syncthreads();
+    if (c == 0) {
+#pragma unroll
+        for (int f = 0; f < F; ++f) st[(size_t)f * 32] = ex[f * 32 + lane];
+    }
+    if (a.carry && ntiles > 1) {
+        float* hn = a.hbuf[ph ^ 1] + (size_t)s * a.Dpad;
+        for (int i = g * blockDim.x + threadIdx.x; i < a.Dpad; i += gridDim.x * blockDim.x) {
+            const int k = a.n - a.Dpad + i;
+            hn[i] = (k >= 0) ? x_s[k] : hist_s[a.n + i];
+        }
+    }
 }
 
 // Several banks that share a lane mapping (F, LPT) in one launch: blockIdx.z picks the bank.  Used by the
@@ -493,7 +707,7 @@ __global__ void spiir_hist_copy_kernel(float* const hbuf0, float* const hbuf1, c
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= S * Dpad) return;
     const int s = i / Dpad, j = i % Dpad;
-    float* cur = (phase_read(phase) ? hbuf1 : hbuf0) + (size_t)s * Dpad;
+    float* cur = (phase_parity(phase) ? hbuf1 : hbuf0) + (size_t)s * Dpad;
     const int k = j - (Dpad - D);                       // index in the caller's row
     if (to_user) { if (k >= 0) user[(size_t)s * D + k] = cur[j]; }
     else cur[j] = k >= 0 ? user[(size_t)s * D + k] : 0.f;

@@ -153,6 +153,8 @@ double layout_conflict_degree(const std::vector<int32_t>& dly, int G, int F)
 // ---------------------------------------------------------------------------------------------
 static inline int round_up(int v, int m) { return (v + m - 1) / m * m; }
 
+bool scan_mapping_supported(int F, int LPT, int NP) { return NP == 1 && F <= 4 && LPT <= 8; }
+
 spiir_status compute_geometry(int T, int L, int S, int Dpad, int n, int opt_chunks, int nc_cap, int n_sm,
                               int smem_optin, FilterGeometry* g)
 {
@@ -163,12 +165,36 @@ spiir_status compute_geometry(int T, int L, int S, int Dpad, int n, int opt_chun
     }
     g->TPG = 32 / g->LPT;
     g->G = g->LPT == 32 ? T * g->NP : (T + g->TPG - 1) / g->TPG;
-    const int kBatch = 16, kMaxWarps = 8;
+    const int kBatch = 16, kMaxWarps = 8, kScanMaxWarps = 16;
+    const int kTileRowBytes = 9 * 16;                      // spiir_filter.cuh: kTileRow4 float4 per store-tile row
     const int kRedWarpBytes = (32 * 9 + 64) * 16;          // spiir_filter.cuh: kRedWarp4 float4 per warp (multi-warp templates)
     // time chunks: only when the bank alone cannot fill the machine
     int NC = 1;
     const long tasks = (long)S * g->G;
     const long target = (long)n_sm * 8;
+    // Few filters per template (several templates per warp, F <= 4): the chunks are the warps of one CTA per warp
+    // task and the carry goes through shared memory -- one launch, so it pays for blocks as short as 64 samples.
+    if (scan_mapping_supported(g->F, g->LPT, g->NP) && opt_chunks != 1 && n >= 64) {
+        long ncw = opt_chunks > 1 ? opt_chunks : (tasks * 2 <= target ? 2 * target / tasks : 1);
+        ncw = std::min<long>(std::min<long>(ncw, kScanMaxWarps), n / 32);
+        if (ncw >= 2) {
+            const int ex_bytes = ((int)ncw + 1) * g->F * 32 * 8 + (g->LPT <= 4 ? (int)ncw * g->TPG * kTileRowBytes : 0);   // chunk states + store tiles
+            const int budget = (smem_optin - 64 - ex_bytes) / 16;
+            int NT = round_up(n, kBatch);
+            if (Dpad + NT + 32 > budget) {                 // several time tiles of equal length
+                const int nt_max = (budget - Dpad - 32) / kBatch * kBatch;
+                const int ntiles = nt_max >= 64 ? (n + nt_max - 1) / nt_max : 0;
+                NT = ntiles ? round_up((n + ntiles - 1) / ntiles, kBatch) : 0;
+            }
+            if (NT >= 64) {
+                const int C = round_up((NT + (int)ncw - 1) / (int)ncw, kBatch);
+                g->scan = 1; g->NC = (NT + C - 1) / C; g->C = C; g->NT = NT; g->CS = Dpad + NT + 32;
+                g->warps = g->NC; g->grid_x = g->G; g->grid_y = S; g->launches = 1;
+                g->smem_bytes = 16 * g->CS + 16 + ex_bytes;
+                return SPIIR_OK;
+            }
+        }
+    }
     if (opt_chunks >= 1) NC = opt_chunks;
     else if (tasks * 2 <= target && n >= 128) {
         // Chunking costs two more launches and 1.75x the arithmetic; it pays only when the time a lone
@@ -195,7 +221,7 @@ spiir_status compute_geometry(int T, int L, int S, int Dpad, int n, int opt_chun
     warps = std::min(warps, g->G);
     if (g->NP > 1) warps = std::max(g->NP, warps / g->NP * g->NP);      // the warps of a template share a CTA
     g->warps = warps;
-    const int red_bytes = g->NP > 1 ? warps * kRedWarpBytes : 0;
+    const int red_bytes = g->NP > 1 ? warps * kRedWarpBytes : (g->LPT <= 4 ? warps * g->TPG * kTileRowBytes : 0);   // or the store tiles
     // time tile: as long as shared memory allows (4 shifted copies of Dpad + NT + 32 floats)
     const int budget_floats = (smem_optin - 64 - red_bytes) / 16;
     int NT = C;

@@ -53,6 +53,7 @@ struct FilterGeometry {
     int warps, grid_x, grid_y;
     int smem_bytes;
     int launches;
+    int scan;                 // NC chunks are the warps of ONE CTA per warp task (spiir_filter_scan_kernel), one launch
 };
 
 constexpr int kMaxFiltersPerTemplate = 2048;
@@ -60,6 +61,7 @@ constexpr int kMaxFiltersPerTemplate = 2048;
 // Pick (F, LPT, NP) for a bank of L filters per template.  Returns false when L is not supported.
 bool choose_lane_mapping(int L, int T, int* F, int* LPT, int* NP);
 int lpt16_min_templates();
+bool scan_mapping_supported(int F, int LPT, int NP);   // spiir_filter_scan_kernel is instantiated for this mapping
 
 // One class of a plan: fills the permuted coefficient / delay arrays ([G][F][32], zero padded) and, for every filter of
 // the listed templates, its index in them.  offsets == nullptr: uniform bank of L filters per template (template t owns

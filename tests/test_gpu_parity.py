@@ -113,6 +113,52 @@ def test_config2_few_filter(sp, oracle_mod, L):
     assert_parity(z, ref, f"cfg2 L={L}")
 
 
+@pytest.mark.parametrize("T,L,S,chunks,blocks", [
+    (70, 1, 1, 0, (256, 256, 37, 1, 64, 300)),          # partially filled last group, ragged blocks, plain fallback below 64
+    (33, 4, 2, 0, (512, 100, 512)),                      # two streams
+    (20, 7, 1, 5, (1000, 333)),                          # two lanes per template, forced chunk count
+    (9, 13, 1, 16, (2048, 2048)),                        # four lanes per template
+    (5, 29, 1, 3, (700, 90, 700)),                       # eight lanes per template
+    (40, 2, 1, 0, (20000, 4000)),                        # block longer than the shared-memory window: several time tiles
+])
+def test_in_cta_time_scan(sp, oracle_mod, T, L, S, chunks, blocks):
+    """Row a7 for the few-filter mappings: the time chunks are the warps of one CTA (spiir_filter_scan_kernel)."""
+    w = _inputs().config(2, n_templates=T, n_filters=L)
+    b = w.banks[0]
+    delays = b.delays.copy()
+    delays.flat[0] = 0
+    delays.flat[-1] = 255
+    plan = sp.Plan(b.a1, b.b0, delays, b.rate_hz, n_streams=S, max_block=max(blocks), time_chunks=chunks)
+    info = plan.launch_info(max(blocks))
+    assert info["launches"] == 1 and info["time_chunks"] > 1, info
+    rng = np.random.default_rng(T * 100 + L)
+    xs = [rng.standard_normal((S, n)).astype(np.float32) for n in blocks]
+    z = stream_gpu_plan(plan, xs)
+    ref = stream_oracle(oracle_mod.FilterOracle(b.a1, b.b0, delays, S), xs)
+    assert_parity(z, ref, f"in-CTA scan T={T} L={L} S={S}")
+    plain = stream_gpu_plan(sp.Plan(b.a1, b.b0, delays, b.rate_hz, n_streams=S, max_block=max(blocks), time_chunks=1), xs)
+    assert_parity(plain, ref, "plain")
+
+
+def test_config2_bulk_call_sampled(sp, oracle_mod):
+    """configs[2] as ONE call of 64 x 256 = 16384 samples (the bulk shape bench.py times), L = 1 and 4: full bank on the
+    GPU, the oracle on templates spread over every CTA (first and last included)."""
+    import torch
+    for L in (1, 4):
+        w = _inputs().config(2, n_filters=L)
+        b = w.banks[0]
+        n = 64 * w.block
+        plan = sp.Plan(b.a1, b.b0, b.delays, b.rate_hz, max_block=n)
+        xs = [np.concatenate([w.strain(k * 64 + i) for i in range(64)], -1) for k in range(2)]
+        idx = np.unique(np.concatenate([np.arange(0, 4096, 37), [31, 32, 4095]]))
+        orc = oracle_mod.FilterOracle(b.a1[idx], b.b0[idx], b.delays[idx])
+        acc = ParityAccumulator()
+        for x in xs:
+            z = plan.filter(torch.from_numpy(x).cuda())
+            acc.add(z[:, torch.from_numpy(idx).cuda()].cpu().numpy(), orc.filter(x))
+        acc.check(f"cfg2 bulk L={L}")
+
+
 # ------------------------------------------------------------------------------------------------
 # config 3: multirate, 7 rates, 192-tap Kaiser resamplers, cascade accumulation
 # ------------------------------------------------------------------------------------------------

@@ -127,13 +127,21 @@ def test_workspace_queries_fail_loudly_without_a_device(sp):
 
 
 def test_chunking_follows_the_cost_model(sp):
-    # configs[2]: 4096 templates x 8 filters, 256-sample blocks -> two more launches never pay
+    # configs[2]: 4096 templates x 1..32 filters, 256-sample blocks -> two more launches never pay; up to 16 filters
+    # (several templates per warp) the chunks are the warps of one CTA: still ONE launch
     for L in (1, 2, 4, 8, 16, 32):
         g = sp.spiir_host_geometry(4096, L, 1, 255, 256)
-        assert g["time_chunks"] == 1 and g["launches"] == 1, L
-    # the two highest rates of configs[3]: 1024 templates x 8 / 16 filters, 4096 / 2048 samples -> chunked
-    assert sp.spiir_host_geometry(1024, 8, 1, 4095, 4096)["time_chunks"] > 1
-    assert sp.spiir_host_geometry(1024, 16, 1, 2047, 2048)["time_chunks"] > 1
+        assert g["launches"] == 1, L
+        assert (g["time_chunks"] > 1) == (L <= 16), (L, g)
+        assert g["time_chunks"] == 1 or g["warps_per_cta"] == g["time_chunks"]
+    assert sp.spiir_host_geometry(4096, 4, 1, 255, 256, time_chunks=1)["time_chunks"] == 1
+    # one bulk call of 16384 samples: equal time tiles that fit the shared-memory window
+    g = sp.spiir_host_geometry(4096, 1, 1, 255, 16384)
+    assert g["launches"] == 1 and g["time_tile"] == 8192 and g["time_chunks"] == 16
+    # the two highest rates of configs[3]: 1024 templates x 8 / 16 filters, 4096 / 2048 samples -> scanned inside a CTA
+    for L, n in ((8, 4096), (16, 2048)):
+        g = sp.spiir_host_geometry(1024, L, 1, n - 1, n)
+        assert g["time_chunks"] > 1 and g["launches"] == 1, (L, g)
     # ... but not its lower rates (one warp per template already gives 1024 warps)
     assert sp.spiir_host_geometry(1024, 32, 1, 1023, 1024)["time_chunks"] == 1
     # a long block of a small bank is chunked, a short one is not
