@@ -155,12 +155,16 @@ spiir_status spiir_kaiser_taps(int n_taps, double kaiser_beta, double cutoff, fl
  *   n_taps even, 2 <= n_taps <= 1024; taps are spiir_kaiser_taps(n_taps, kaiser_beta, cutoff).
  *   Register-blocked kernels exist for 384 / 192 / 32 taps (the paper's 384-tap
  *   down and 32-tap up filters; configs[3]: 192), a generic kernel serves every other count.
- *   opts: NULL means {4096, NULL, 0}.
+ *   The 192-tap up stage of a large call (rows * n_in >= 65536) runs on the tensor cores: the polyphase FIR as
+ *   a banded-Toeplitz contraction, tcgen05 kind::tf32 with every operand split into a TF32-exact high part and
+ *   its float32 remainder, three passes accumulated in TMEM (float32-level accuracy).
+ *   opts: NULL means {4096, NULL, 0, 0}.
  * ------------------------------------------------------------------------------------------- */
 typedef struct {
     int    max_block;        /* largest n_in of a call */
     void*  workspace;        /* DEVICE, caller-owned; NULL: the library allocates */
     size_t workspace_bytes;
+    int    flags;            /* bit 0: never use the tensor-core kernel (192-tap up stage), for A/B measurements */
 } spiir_resamp_opts;
 
 size_t       spiir_resamp_workspace_bytes(int direction, int n_taps, int n_rows);

@@ -50,7 +50,8 @@ class _PlanOpts(ctypes.Structure):
 
 
 class _ResampOpts(ctypes.Structure):
-    _fields_ = [("max_block", ctypes.c_int), ("workspace", ctypes.c_void_p), ("workspace_bytes", ctypes.c_size_t)]
+    _fields_ = [("max_block", ctypes.c_int), ("workspace", ctypes.c_void_p), ("workspace_bytes", ctypes.c_size_t),
+                ("flags", ctypes.c_int)]
 
 
 class _MrOpts(ctypes.Structure):
@@ -336,12 +337,12 @@ class Resampler:
     """One streaming x2 stage (spiir_resamp_create / spiir_resample_down / spiir_resample_up)."""
 
     def __init__(self, direction: str, n_rows: int, max_block: int, n_taps: int = 192, kaiser_beta: float = 5.0,
-                 cutoff: float = 0.25):
+                 cutoff: float = 0.25, flags: int = 0):
         self.direction, self.rows, self.max_block = direction, int(n_rows), int(max_block)
         code = {"down": SPIIR_DOWN2, "up": SPIIR_UP2}[direction]
         need = lib().spiir_resamp_workspace_bytes(code, int(n_taps), self.rows)
         self._ws = _workspace(need) if need else None
-        opts = _ResampOpts(self.max_block, self._ws.data_ptr() if self._ws is not None else None, need)
+        opts = _ResampOpts(self.max_block, self._ws.data_ptr() if self._ws is not None else None, need, int(flags))
         self._h = ctypes.c_void_p()
         _check(lib().spiir_resamp_create(ctypes.byref(self._h), code, n_taps, kaiser_beta, cutoff, self.rows,
                                          ctypes.byref(opts)), "spiir_resamp_create")

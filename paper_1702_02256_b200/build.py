@@ -15,7 +15,6 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libspiir.so")
 SOURCES = ["spiir_api.cu", "spiir_resamp.cu", "spiir_mr.cu", "spiir_probe.cu", "spiir_paper_design.cu", "spiir_host.cpp"]
-HEADERS = ["spiir_filter.cuh", "spiir_resample.cuh", "spiir_common.cuh", "spiir_internal.h", os.path.join("..", "..", "include", "spiir.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "--use_fast_math=false"]
 
@@ -31,8 +30,12 @@ def needs_build() -> bool:
     if not os.path.exists(LIB):
         return True
     t = os.path.getmtime(LIB)
-    deps = [os.path.join(CSRC, s) for s in SOURCES + HEADERS] + [os.path.abspath(__file__)]
-    return any(os.path.getmtime(d) > t for d in deps)
+    for s in SOURCES:
+        src = os.path.join(CSRC, s)
+        deps = [src, os.path.abspath(__file__)] + sorted(_includes(src))
+        if any(os.path.exists(d) and os.path.getmtime(d) > t for d in deps):
+            return True
+    return False
 
 
 def _includes(path: str, seen=None) -> set:

@@ -114,6 +114,8 @@ struct spiir_resamp {
     int direction = 0, N = 0, rows = 0, max_block = 0;
     int H = 0;                        // history samples per row
     float* d_taps = nullptr;
+    float* d_bmat = nullptr;          // up stage, 192 taps: Toeplitz operand of the tensor-core FIR (hi, lo parts)
+    int flags = 0;                    // spiir_resamp_opts.flags
     void* d_hist[2] = {nullptr, nullptr};
     int* d_phase = nullptr;           // {phase, arrivals}
     std::vector<float> taps;
@@ -130,7 +132,7 @@ spiir_status filter_launch_group(spiir_plan* const* ps, const float* const* xs, 
                                  cudaStream_t st);
 int plan_launches(const spiir_plan* p, int n);
 spiir_status resamp_create_in(spiir_resamp_t** out, int direction, int n_taps, double kaiser_beta, double cutoff, int n_rows,
-                              int max_block, Arena* parent);
+                              int max_block, Arena* parent, int flags = 0);
 spiir_status plan_create_in(spiir_plan_t** out, const spiir_c64* a1, const spiir_c64* b0, const int32_t* delays,
                             const int32_t* offsets, int n_templates, int n_filters, int rate_hz, const spiir_plan_opts& o,
                             Arena* parent);

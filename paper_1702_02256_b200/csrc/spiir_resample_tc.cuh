@@ -1,0 +1,342 @@
+// spiir_resample_tc.cuh -- up-by-2 (+ accumulate) with the 192-tap FIR on the 5th-generation tensor cores
+// (row a10 of SURVEY.md section 8; Eq. 9).
+//
+// The polyphase FIR  w[2m+p] = 2 sum_{q<96} h[2q+p] v[m-q]  of a strip of 64 complex rows is a dense contraction
+// with a banded Toeplitz matrix, one tile = 64 input positions -> 128 outputs:
+//     D[t, row'] = sum_k T[t, k] * X[row', k]
+//   T: 128 outputs of the tile x a window of K = 160 input samples (96 before the tile + its 64 inputs),
+//      T[2m'+p, k] = 2 h[2 (96 + m' - k) + p] for 1 <= k - m' <= 96, zero elsewhere (60 % dense).  It is the same for
+//      every tile, so it lives in TENSOR MEMORY for the whole kernel (the A operand of tcgen05.mma may come from TMEM);
+//   X: 128 real rows (re of the 64 rows, then im) x the window, the DATA, in shared memory (B operand, K-major);
+//   D: 128 lanes (outputs) x 128 columns (real rows) of float32 in TMEM.
+// tcgen05.mma kind::tf32 (M = 128, N = 128, K = 8 per instruction: measured 67 cycles, i.e. the nominal TF32 rate;
+// N <= 64 costs the same 55 cycles per instruction, so narrow tiles waste the pipe).  One TF32 pass has 2^-11
+// input precision, far outside the 1e-5 tolerance: every operand is split into a TF32-exact high part and the
+// float32 remainder and three passes are accumulated, T_hi X_hi + T_lo X_hi + T_hi X_lo (the dropped T_lo X_lo
+// term is 2^-22 relative).
+//
+// The data operand uses the canonical K-major, non-swizzled layout: 16-byte "units" of 4 consecutive samples,
+// unit u of real row r at u * 2048 + r * 16.  It is a RING of 48 units (6 chunks of 32 samples): a tile's window
+// is 5 consecutive chunks, every tile advances it by two, so each input sample is written to shared memory once
+// and read by 2.5 tiles; a K = 8 instruction takes two adjacent units and never straddles the ring's end.
+//
+// Roles (416 threads): warps 0-3 load + split + store the data chunks (global loads prefetched two chunks deep in
+// registers), warp 12 issues the MMAs (one thread) and owns TMEM, warps 4-11 drain the accumulator (tcgen05.ld):
+// a lane is an output sample, so a warp writes 256 contiguous bytes of one row per store -- no transposition; with
+// accumulate the store is a vector reduction (red.global.add.v2.f32) done by the L2.  mbarriers: full[6] /
+// empty[6] per ring chunk, tfull / tempty for the accumulator.  CTAs are persistent over (strip, time segment) units.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "spiir_common.cuh"
+
+namespace spiir {
+namespace tc {
+
+constexpr int ROWS = 64;                       // complex rows per strip
+constexpr int NR = 2 * ROWS;                   // real rows = UMMA N
+constexpr int TIN = 64;                        // input samples per tile
+constexpr int MOUT = 2 * TIN;                  // outputs per tile = UMMA M
+constexpr int HALF = 96;                       // taps per polyphase branch (192-tap filter)
+constexpr int KWIN = HALF + TIN;               // 160
+constexpr int KSTEPS = KWIN / 8;               // 20 MMA k-steps per pass
+constexpr int CHS = 32;                        // samples per chunk
+constexpr int CHU = CHS / 4;                   // units per chunk
+constexpr int WIN_CH = KWIN / CHS;             // 5 chunks per window
+constexpr int HALO_CH = HALF / CHS;            // 3 chunks in front of the first tile of a unit
+constexpr int RING_CH = WIN_CH + 1;            // one chunk of prefetch space
+constexpr int RING_UNITS = RING_CH * CHU;      // 48 (even)
+constexpr int UNIT_BYTES = NR * 16;
+constexpr int PART_BYTES = RING_UNITS * UNIT_BYTES;
+constexpr int OFF_LO = PART_BYTES;
+constexpr int OFF_BAR = 2 * PART_BYTES;
+constexpr int NBAR = 2 * RING_CH + 2;
+constexpr int OFF_TPTR = OFF_BAR + NBAR * 8;
+constexpr int SMEM_BYTES = OFF_TPTR + 16;
+constexpr int THREADS = 416;                   // 4 loader warps, 8 epilogue warps, 1 MMA warp
+constexpr int PREFETCH = 2;                    // chunks of global loads in flight per loader thread
+constexpr int TMEM_COLS = 512;
+constexpr int COL_THI = 0, COL_TLO = KWIN, COL_D = 384;
+constexpr int TMAT_FLOATS = 2 * MOUT * KWIN;   // T_hi then T_lo, [128][160] each
+
+struct UpTcArgs {
+    const float2* in;        // [rows][n_in]
+    float2*       out;       // [rows][2 n_in]
+    float2*       hbuf[2];   // [rows][95] ping-pong history
+    int*          phase;
+    const float*  tmat;      // DEVICE: T_hi [128][160] then T_lo [128][160]
+    int rows, n_in, accumulate;
+    int nstrips, nsegs, seg_tiles, tiles_per_row;
+    int in16;                // rows of `in` are 16-byte aligned
+};
+
+__device__ __forceinline__ uint32_t s32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void bar_init(uint32_t bar, int count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
+}
+__device__ __forceinline__ void bar_arrive(uint32_t bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+// Bounded spin: a protocol error becomes a trap (a CUDA error the caller sees), never a hung GPU.
+__device__ __forceinline__ void bar_wait(uint32_t bar, uint32_t parity)
+{
+    for (int it = 0; it < (1 << 28); ++it) {
+        uint32_t ok;
+        asm volatile("{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}"
+                     : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+        if (ok) return;
+    }
+    __trap();
+}
+__device__ __forceinline__ uint64_t smem_desc(uint32_t addr, uint32_t lbo, uint32_t sbo)
+{
+    // K-major, no swizzle: start address, leading (K) and stride (8-row group) byte offsets in 16-byte units, version 1
+    return (uint64_t)((addr >> 4) & 0x3fff) | ((uint64_t)((lbo >> 4) & 0x3fff) << 16) | ((uint64_t)((sbo >> 4) & 0x3fff) << 32) |
+           ((uint64_t)1 << 46);
+}
+// D[tmem_d] (+)= A[tmem_a] * B[smem descriptor]: the A operand (the Toeplitz matrix) is read from tensor memory
+__device__ __forceinline__ void umma_tf32_ts(uint32_t tmem_d, uint32_t tmem_a, uint64_t bdesc, uint32_t idesc, uint32_t accumulate)
+{
+    asm volatile("{\n .reg .pred p;\n setp.ne.b32 p, %4, 0;\n"
+                 " tcgen05.mma.cta_group::1.kind::tf32 [%0], [%1], %2, %3, {%5, %5, %5, %5}, p;\n}"
+                 ::"r"(tmem_d), "r"(tmem_a), "l"(bdesc), "r"(idesc), "r"(accumulate), "r"(0u) : "memory");
+}
+// 32 consecutive columns of this thread's TMEM lane <-> 32 registers
+__device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&v)[32])
+{
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x32.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
+                 "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
+                 : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
+                   "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15]),
+                   "=r"(v[16]), "=r"(v[17]), "=r"(v[18]), "=r"(v[19]), "=r"(v[20]), "=r"(v[21]), "=r"(v[22]), "=r"(v[23]),
+                   "=r"(v[24]), "=r"(v[25]), "=r"(v[26]), "=r"(v[27]), "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
+                 : "r"(taddr));
+}
+__device__ __forceinline__ void tmem_st32(uint32_t taddr, const uint32_t (&v)[32])
+{
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x32.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16, "
+                 "%17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31, %32};"
+                 ::"r"(taddr), "r"(v[0]), "r"(v[1]), "r"(v[2]), "r"(v[3]), "r"(v[4]), "r"(v[5]), "r"(v[6]), "r"(v[7]),
+                   "r"(v[8]), "r"(v[9]), "r"(v[10]), "r"(v[11]), "r"(v[12]), "r"(v[13]), "r"(v[14]), "r"(v[15]),
+                   "r"(v[16]), "r"(v[17]), "r"(v[18]), "r"(v[19]), "r"(v[20]), "r"(v[21]), "r"(v[22]), "r"(v[23]),
+                   "r"(v[24]), "r"(v[25]), "r"(v[26]), "r"(v[27]), "r"(v[28]), "r"(v[29]), "r"(v[30]), "r"(v[31]) : "memory");
+}
+__device__ __forceinline__ void umma_commit(uint32_t bar)
+{
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ float tf32_hi(float x)
+{
+    uint32_t r;
+    asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(r) : "f"(x));
+    return __uint_as_float(r);
+}
+
+// sample m of a row (m relative to the block): history for -95 <= m < 0, zero outside
+__device__ __forceinline__ float2 sample_at(const float2* in_row, const float2* hist_row, int m, int n_in)
+{
+    if (m >= 0) return m < n_in ? in_row[m] : make_float2(0.f, 0.f);
+    return m >= -(HALF - 1) ? hist_row[HALF - 1 + m] : make_float2(0.f, 0.f);
+}
+
+
+__global__ void __launch_bounds__(THREADS, 1) spiir_up2_tc_kernel(const UpTcArgs a)
+{
+    extern __shared__ __align__(1024) unsigned char sm[];
+    const uint32_t sbase = s32(sm);
+    const uint32_t bar0 = sbase + OFF_BAR;
+    auto full = [&](int i) { return bar0 + 8u * (uint32_t)i; };
+    auto empty = [&](int i) { return bar0 + 8u * (uint32_t)(RING_CH + i); };
+    const uint32_t tfull = bar0 + 8u * (uint32_t)(2 * RING_CH), tempty = tfull + 8u;
+    uint32_t* tptr = reinterpret_cast<uint32_t*>(sm + OFF_TPTR);
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int ph = phase_read(a.phase);
+    const float2* hcur = a.hbuf[ph];
+    float2* hnext = a.hbuf[ph ^ 1];
+
+    // ---- one-time setup: barriers, tensor memory, the Toeplitz operand into TMEM --------------------------
+    if (tid == 0) {
+        for (int i = 0; i < RING_CH; ++i) { bar_init(full(i), 128); bar_init(empty(i), 1); }
+        bar_init(tfull, 1);
+        bar_init(tempty, 256);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (warp == 12) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(s32(tptr)), "r"(TMEM_COLS));
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::);
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    const uint32_t tmem = *tptr;
+    if (warp >= 4 && warp < 8) {                                       // lane t of TMEM = output t of a tile
+        const int t = (warp & 3) * 32 + lane;
+        const uint32_t lane_addr = tmem + ((uint32_t)((warp & 3) * 32) << 16);
+        for (int part = 0; part < 2; ++part) {
+            const float* src = a.tmat + ((size_t)part * MOUT + t) * KWIN;
+            for (int c0 = 0; c0 < KWIN; c0 += 32) {
+                uint32_t v[32];
+#pragma unroll
+                for (int i = 0; i < 32; ++i) v[i] = __float_as_uint(src[c0 + i]);
+                tmem_st32(lane_addr + (uint32_t)(part ? COL_TLO : COL_THI) + (uint32_t)c0, v);
+            }
+        }
+        asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+
+    const int nunits = a.nstrips * a.nsegs;
+    int cbase = 0, tbase = 0;                                          // chunks / tiles of this CTA's earlier units
+    for (int u = blockIdx.x; u < nunits; u += gridDim.x) {
+        const int strip = u / a.nsegs, seg = u % a.nsegs;
+        const int tile0 = seg * a.seg_tiles;
+        const int J = min(a.seg_tiles, a.tiles_per_row - tile0);
+        const int ms = tile0 * TIN;
+        const int row0 = strip * ROWS;
+        const int nch = WIN_CH - 2 + 2 * J;                            // chunks of this unit: 3 of halo + 2 per tile
+
+        if (warp < 4) {
+            // ===== loaders: 64 rows x 32 samples per chunk; thread = (row, 16 samples = 4 units) =====
+            const int r = (warp & 1) * 32 + lane, hsel = warp >> 1;
+            const int row = row0 + r;
+            const bool rowok = row < a.rows;
+            const float2* in_row = a.in + (size_t)(rowok ? row : 0) * a.n_in;
+            const float2* hist_row = hcur + (size_t)(rowok ? row : 0) * (HALF - 1);
+            if (seg == 0) {
+                // carried history of this strip's rows: the last 95 samples of (history ++ block)
+                for (int i = tid; i < ROWS * (HALF - 1); i += 128) {
+                    const int rr = i / (HALF - 1), k = i % (HALF - 1), rw = row0 + rr;
+                    if (rw < a.rows) {
+                        const int g = a.n_in - (HALF - 1) + k;
+                        hnext[(size_t)rw * (HALF - 1) + k] =
+                            g >= 0 ? a.in[(size_t)rw * a.n_in + g] : hcur[(size_t)rw * (HALF - 1) + a.n_in + k];
+                    }
+                }
+            }
+            for (int c0 = 0; c0 < nch; c0 += PREFETCH) {
+                float4 q[PREFETCH][8];                                  // 16 complex samples per chunk and thread
+#pragma unroll
+                for (int pi = 0; pi < PREFETCH; ++pi) {
+                    const int ci = c0 + pi;
+                    const int m = ms - HALF + ci * CHS + hsel * 16;
+                    if (ci < nch && rowok && m >= 0 && m + 16 <= a.n_in && a.in16) {
+                        const float4* p = reinterpret_cast<const float4*>(in_row + m);
+#pragma unroll
+                        for (int i = 0; i < 8; ++i) q[pi][i] = p[i];
+                    } else {
+#pragma unroll
+                        for (int i = 0; i < 8; ++i) {
+                            float2 s0 = make_float2(0.f, 0.f), s1 = s0;
+                            if (ci < nch && rowok) { s0 = sample_at(in_row, hist_row, m + 2 * i, a.n_in); s1 = sample_at(in_row, hist_row, m + 2 * i + 1, a.n_in); }
+                            q[pi][i] = make_float4(s0.x, s0.y, s1.x, s1.y);
+                        }
+                    }
+                }
+#pragma unroll
+                for (int pi = 0; pi < PREFETCH; ++pi) {
+                    const int ci = c0 + pi;
+                    if (ci < nch) {
+                        const int c = cbase + ci, slot = c % RING_CH, fill = c / RING_CH;
+                        if (fill > 0) bar_wait(empty(slot), (uint32_t)((fill - 1) & 1));
+#pragma unroll
+                        for (int uu = 0; uu < 4; ++uu) {
+                            const float4 s01 = q[pi][2 * uu], s23 = q[pi][2 * uu + 1];
+                            const float4 re = make_float4(s01.x, s01.z, s23.x, s23.z), im = make_float4(s01.y, s01.w, s23.y, s23.w);
+                            const float4 reh = make_float4(tf32_hi(re.x), tf32_hi(re.y), tf32_hi(re.z), tf32_hi(re.w));
+                            const float4 imh = make_float4(tf32_hi(im.x), tf32_hi(im.y), tf32_hi(im.z), tf32_hi(im.w));
+                            const float4 rel = make_float4(re.x - reh.x, re.y - reh.y, re.z - reh.z, re.w - reh.w);
+                            const float4 iml = make_float4(im.x - imh.x, im.y - imh.y, im.z - imh.z, im.w - imh.w);
+                            unsigned char* unit = sm + (size_t)(slot * CHU + hsel * 4 + uu) * UNIT_BYTES;
+                            *reinterpret_cast<float4*>(unit + r * 16) = reh;
+                            *reinterpret_cast<float4*>(unit + (ROWS + r) * 16) = imh;
+                            *reinterpret_cast<float4*>(unit + OFF_LO + r * 16) = rel;
+                            *reinterpret_cast<float4*>(unit + OFF_LO + (ROWS + r) * 16) = iml;
+                        }
+                        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+                        bar_arrive(full(slot));
+                    }
+                }
+            }
+        } else
+        if (warp == 12) {
+            // ===== MMA issuer (one thread) =====
+            if (lane == 0) {
+                const uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(NR >> 3) << 17) | ((uint32_t)(MOUT >> 4) << 24);
+                const uint32_t d = tmem + COL_D;
+                for (int j = 0; j < J; ++j) {
+                    const int cn = cbase + 2 * j + WIN_CH - 1;          // newest chunk of this tile's window
+                    bar_wait(full(cn % RING_CH), (uint32_t)((cn / RING_CH) & 1));
+                    const int t = tbase + j;
+                    if (t > 0) bar_wait(tempty, (uint32_t)((t - 1) & 1));   // the previous tile's accumulator has been read
+                    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+                    const int wu0 = ((cbase + 2 * j) % RING_CH) * CHU;  // ring unit of the window's first unit
+#pragma unroll 2
+                    for (int ks = 0; ks < KSTEPS; ++ks) {
+                        int ru = wu0 + 2 * ks;
+                        if (ru >= RING_UNITS) ru -= RING_UNITS;
+                        const uint32_t x_hi = sbase + (uint32_t)ru * UNIT_BYTES;
+                        const uint64_t dxh = smem_desc(x_hi, UNIT_BYTES, 128), dxl = smem_desc(x_hi + OFF_LO, UNIT_BYTES, 128);
+                        const uint32_t thi = tmem + COL_THI + (uint32_t)(8 * ks), tlo = tmem + COL_TLO + (uint32_t)(8 * ks);
+                        umma_tf32_ts(d, thi, dxh, idesc, ks > 0 ? 1u : 0u);
+                        umma_tf32_ts(d, tlo, dxh, idesc, 1u);
+                        umma_tf32_ts(d, thi, dxl, idesc, 1u);
+                    }
+                    umma_commit(empty((cbase + 2 * j) % RING_CH));     // the window's two oldest chunks are free once these MMAs are done
+                    umma_commit(empty((cbase + 2 * j + 1) % RING_CH));
+                    umma_commit(tfull);
+                }
+                for (int i = 0; i < HALO_CH; ++i) umma_commit(empty((cbase + 2 * J + i) % RING_CH));
+            }
+            __syncwarp();
+        } else {
+            // ===== epilogue, 256 threads: TMEM lane = output sample, columns = real rows.  Warp group `half` takes the
+            // complex rows [32 half, 32 half + 32): re in columns 32 half.., im in columns 64 + 32 half.. =====
+            const int ew = warp & 3, half = (warp - 4) >> 2;
+            const int tl = ew * 32 + lane;                              // output index within the tile
+            const uint32_t taddr = tmem + ((uint32_t)(ew * 32) << 16) + COL_D + (uint32_t)(32 * half);
+            for (int j = 0; j < J; ++j) {
+                const int t = tbase + j;
+                const int m0 = ms + j * TIN;
+                const bool tok = tl < 2 * min(TIN, a.n_in - m0);
+                float2* obase = a.out + (size_t)(row0 + 32 * half) * 2 * a.n_in + 2 * m0 + tl;
+                bar_wait(tfull, (uint32_t)(t & 1));
+                asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+                uint32_t vre[32], vim[32];
+                tmem_ld32(taddr, vre);
+                tmem_ld32(taddr + ROWS, vim);
+                asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+                asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+                bar_arrive(tempty);                                     // the accumulator may be overwritten
+                // accumulate = a vector reduction performed by the L2 (one addend per element and call: deterministic); no
+                // read-modify-write round trip through this thread's registers
+                if (a.accumulate) {
+#pragma unroll
+                    for (int i = 0; i < 32; ++i)
+                        if (tok && row0 + 32 * half + i < a.rows)
+                            asm volatile("red.global.add.v2.f32 [%0], {%1, %2};" ::"l"(obase + (size_t)i * 2 * a.n_in),
+                                         "f"(__uint_as_float(vre[i])), "f"(__uint_as_float(vim[i])) : "memory");
+                } else {
+#pragma unroll
+                    for (int i = 0; i < 32; ++i)
+                        if (tok && row0 + 32 * half + i < a.rows)
+                            obase[(size_t)i * 2 * a.n_in] = make_float2(__uint_as_float(vre[i]), __uint_as_float(vim[i]));
+                }
+            }
+        }
+        cbase += nch;
+        tbase += J;
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    const bool last = last_cta_arrives(a.phase, gridDim.x);           // __syncthreads inside
+    if (last) a.phase[0] = ph ^ 1;
+    if (warp == 12) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"(TMEM_COLS));
+}
+
+}  // namespace tc
+}  // namespace spiir
