@@ -20,8 +20,8 @@
 // is 5 consecutive chunks, every tile advances it by two, so each input sample is written to shared memory once
 // and read by 2.5 tiles; a K = 8 instruction takes two adjacent units and never straddles the ring's end.
 //
-// Roles (416 threads): warps 0-3 load + split + store the data chunks (global loads prefetched two chunks deep in
-// registers), warp 12 issues the MMAs (one thread) and owns TMEM, warps 4-11 drain the accumulator (tcgen05.ld):
+// Roles (416 threads): warps 0-7 load + split + store the data chunks (global loads prefetched four chunks deep in
+// registers: 64 KB in flight per SM), warp 12 issues the MMAs (one thread) and owns TMEM, warps 8-11 drain the accumulator (tcgen05.ld):
 // a lane is an output sample, so a warp writes 256 contiguous bytes of one row per store -- no transposition; with
 // accumulate the store is a vector reduction (red.global.add.v2.f32) done by the L2.  mbarriers: full[6] /
 // empty[6] per ring chunk, tfull / tempty for the accumulator.  CTAs are persistent over (strip, time segment) units.
@@ -33,6 +33,14 @@
 
 namespace spiir {
 namespace tc {
+#ifdef SPIIR_TC_DEBUG
+__device__ long long g_dbg[16];
+#define TC_T0 const long long t0__ = clock64();
+#define TC_ACC(i) if (blockIdx.x == 0) atomicAdd((unsigned long long*)&g_dbg[i], (unsigned long long)(clock64() - t0__));
+#else
+#define TC_T0
+#define TC_ACC(i)
+#endif
 
 constexpr int ROWS = 64;                       // complex rows per strip
 constexpr int NR = 2 * ROWS;                   // real rows = UMMA N
@@ -54,8 +62,10 @@ constexpr int OFF_BAR = 2 * PART_BYTES;
 constexpr int NBAR = 2 * RING_CH + 2;
 constexpr int OFF_TPTR = OFF_BAR + NBAR * 8;
 constexpr int SMEM_BYTES = OFF_TPTR + 16;
-constexpr int THREADS = 416;                   // 4 loader warps, 8 epilogue warps, 1 MMA warp
-constexpr int PREFETCH = 2;                    // chunks of global loads in flight per loader thread
+constexpr int LOADER_WARPS = 8;
+constexpr int EPI_WARPS = 4;
+constexpr int THREADS = (LOADER_WARPS + EPI_WARPS + 1) * 32;   // loader warps, epilogue warps, 1 MMA warp (416: 128 registers each)
+constexpr int PREFETCH = 4;                    // chunks of global loads in flight per loader thread (64 KB per CTA)
 constexpr int TMEM_COLS = 512;
 constexpr int COL_THI = 0, COL_TLO = KWIN, COL_D = 384;
 constexpr int TMAT_FLOATS = 2 * MOUT * KWIN;   // T_hi then T_lo, [128][160] each
@@ -116,6 +126,13 @@ __device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&v)[32])
                    "=r"(v[24]), "=r"(v[25]), "=r"(v[26]), "=r"(v[27]), "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
                  : "r"(taddr));
 }
+__device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t (&v)[16])
+{
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
+                 : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
+                   "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
+                 : "r"(taddr));
+}
 __device__ __forceinline__ void tmem_st32(uint32_t taddr, const uint32_t (&v)[32])
 {
     asm volatile("tcgen05.st.sync.aligned.32x32b.x32.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16, "
@@ -124,6 +141,10 @@ __device__ __forceinline__ void tmem_st32(uint32_t taddr, const uint32_t (&v)[32
                    "r"(v[8]), "r"(v[9]), "r"(v[10]), "r"(v[11]), "r"(v[12]), "r"(v[13]), "r"(v[14]), "r"(v[15]),
                    "r"(v[16]), "r"(v[17]), "r"(v[18]), "r"(v[19]), "r"(v[20]), "r"(v[21]), "r"(v[22]), "r"(v[23]),
                    "r"(v[24]), "r"(v[25]), "r"(v[26]), "r"(v[27]), "r"(v[28]), "r"(v[29]), "r"(v[30]), "r"(v[31]) : "memory");
+}
+__device__ __forceinline__ void sts128(uint32_t addr, float4 v)
+{
+    asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w) : "memory");
 }
 __device__ __forceinline__ void umma_commit(uint32_t bar)
 {
@@ -160,12 +181,12 @@ __global__ void __launch_bounds__(THREADS, 1) spiir_up2_tc_kernel(const UpTcArgs
 
     // ---- one-time setup: barriers, tensor memory, the Toeplitz operand into TMEM --------------------------
     if (tid == 0) {
-        for (int i = 0; i < RING_CH; ++i) { bar_init(full(i), 128); bar_init(empty(i), 1); }
+        for (int i = 0; i < RING_CH; ++i) { bar_init(full(i), LOADER_WARPS * 32); bar_init(empty(i), 1); }
         bar_init(tfull, 1);
-        bar_init(tempty, 256);
+        bar_init(tempty, EPI_WARPS * 32);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
-    if (warp == 12) {
+    if (warp == LOADER_WARPS + EPI_WARPS) {
         asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(s32(tptr)), "r"(TMEM_COLS));
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::);
     }
@@ -173,7 +194,7 @@ __global__ void __launch_bounds__(THREADS, 1) spiir_up2_tc_kernel(const UpTcArgs
     __syncthreads();
     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
     const uint32_t tmem = *tptr;
-    if (warp >= 4 && warp < 8) {                                       // lane t of TMEM = output t of a tile
+    if (warp >= LOADER_WARPS && warp < LOADER_WARPS + 4) {             // lane t of TMEM = output t of a tile
         const int t = (warp & 3) * 32 + lane;
         const uint32_t lane_addr = tmem + ((uint32_t)((warp & 3) * 32) << 16);
         for (int part = 0; part < 2; ++part) {
@@ -201,16 +222,25 @@ __global__ void __launch_bounds__(THREADS, 1) spiir_up2_tc_kernel(const UpTcArgs
         const int row0 = strip * ROWS;
         const int nch = WIN_CH - 2 + 2 * J;                            // chunks of this unit: 3 of halo + 2 per tile
 
-        if (warp < 4) {
-            // ===== loaders: 64 rows x 32 samples per chunk; thread = (row, 16 samples = 4 units) =====
-            const int r = (warp & 1) * 32 + lane, hsel = warp >> 1;
+        if (warp < LOADER_WARPS) {
+            // ===== loaders: 64 rows x 32 samples per chunk.  A warp owns 8 rows; lane = (row, piece): every load instruction
+            // reads 4 consecutive 16-byte pieces (64 contiguous bytes) of each of its 8 rows, so the L1 sees 8 line requests
+            // per instruction instead of 32.  A piece is two samples = half a unit: lane pairs (piece, piece ^ 1) swap halves
+            // so that the even lane ends up with re[4] and the odd lane with im[4] of one unit; a quarter warp then stores
+            // 8 different rows of one unit: conflict-free 16-byte stores. =====
+            const int rowlow = lane & 7, piece = lane >> 3;
+            const int r = warp * 8 + rowlow;
+            const bool odd = (piece & 1) != 0;
             const int row = row0 + r;
             const bool rowok = row < a.rows;
             const float2* in_row = a.in + (size_t)(rowok ? row : 0) * a.n_in;
             const float2* hist_row = hcur + (size_t)(rowok ? row : 0) * (HALF - 1);
-            if (seg == 0) {
-                // carried history of this strip's rows: the last 95 samples of (history ++ block)
-                for (int i = tid; i < ROWS * (HALF - 1); i += 128) {
+            // Carried history of this strip's rows = the last 95 samples of (history ++ block).  A block of at least 95 samples
+            // supplies all of them, and they pass through this thread's registers anyway (written below); shorter blocks
+            // take this explicit copy.
+            const int hfirst = a.n_in - (HALF - 1);                     // first block sample that is part of the next history
+            if (seg == 0 && hfirst < 0) {
+                for (int i = tid; i < ROWS * (HALF - 1); i += LOADER_WARPS * 32) {
                     const int rr = i / (HALF - 1), k = i % (HALF - 1), rw = row0 + rr;
                     if (rw < a.rows) {
                         const int g = a.n_in - (HALF - 1) + k;
@@ -219,63 +249,73 @@ __global__ void __launch_bounds__(THREADS, 1) spiir_up2_tc_kernel(const UpTcArgs
                     }
                 }
             }
-            for (int c0 = 0; c0 < nch; c0 += PREFETCH) {
-                float4 q[PREFETCH][8];                                  // 16 complex samples per chunk and thread
+            // rolling software prefetch: the loads of chunk ci + PREFETCH are issued as soon as chunk ci's registers
+            // have been consumed, so PREFETCH chunks stay in flight while this thread waits for ring space
+            float4 q[PREFETCH][4];                                      // pieces piece, piece + 4, piece + 8, piece + 12 of the chunk
+            auto issue = [&](int ci, float4 (&dst)[4]) {
+                const int mc = ms - HALF + ci * CHS;                    // first sample of the chunk
+                if (ci < nch && rowok && mc >= 0 && mc + CHS <= a.n_in && a.in16) {
+                    const float4* p = reinterpret_cast<const float4*>(in_row + mc) + piece;
 #pragma unroll
-                for (int pi = 0; pi < PREFETCH; ++pi) {
-                    const int ci = c0 + pi;
-                    const int m = ms - HALF + ci * CHS + hsel * 16;
-                    if (ci < nch && rowok && m >= 0 && m + 16 <= a.n_in && a.in16) {
-                        const float4* p = reinterpret_cast<const float4*>(in_row + m);
+                    for (int i = 0; i < 4; ++i) dst[i] = p[4 * i];
+                } else {
 #pragma unroll
-                        for (int i = 0; i < 8; ++i) q[pi][i] = p[i];
-                    } else {
-#pragma unroll
-                        for (int i = 0; i < 8; ++i) {
-                            float2 s0 = make_float2(0.f, 0.f), s1 = s0;
-                            if (ci < nch && rowok) { s0 = sample_at(in_row, hist_row, m + 2 * i, a.n_in); s1 = sample_at(in_row, hist_row, m + 2 * i + 1, a.n_in); }
-                            q[pi][i] = make_float4(s0.x, s0.y, s1.x, s1.y);
-                        }
+                    for (int i = 0; i < 4; ++i) {
+                        float2 s0 = make_float2(0.f, 0.f), s1 = s0;
+                        const int m = mc + 2 * (4 * i + piece);
+                        if (ci < nch && rowok) { s0 = sample_at(in_row, hist_row, m, a.n_in); s1 = sample_at(in_row, hist_row, m + 1, a.n_in); }
+                        dst[i] = make_float4(s0.x, s0.y, s1.x, s1.y);
                     }
                 }
+            };
+#pragma unroll
+            for (int pi = 0; pi < PREFETCH; ++pi) issue(pi, q[pi]);
+            for (int c0 = 0; c0 < nch; c0 += PREFETCH) {
 #pragma unroll
                 for (int pi = 0; pi < PREFETCH; ++pi) {
                     const int ci = c0 + pi;
-                    if (ci < nch) {
+                    if (ci < nch) {                                      // uniform over the CTA's loader threads
                         const int c = cbase + ci, slot = c % RING_CH, fill = c / RING_CH;
-                        if (fill > 0) bar_wait(empty(slot), (uint32_t)((fill - 1) & 1));
+                        { TC_T0 if (fill > 0) bar_wait(empty(slot), (uint32_t)((fill - 1) & 1)); if (tid == 0) { TC_ACC(3) } }
 #pragma unroll
-                        for (int uu = 0; uu < 4; ++uu) {
-                            const float4 s01 = q[pi][2 * uu], s23 = q[pi][2 * uu + 1];
-                            const float4 re = make_float4(s01.x, s01.z, s23.x, s23.z), im = make_float4(s01.y, s01.w, s23.y, s23.w);
-                            const float4 reh = make_float4(tf32_hi(re.x), tf32_hi(re.y), tf32_hi(re.z), tf32_hi(re.w));
-                            const float4 imh = make_float4(tf32_hi(im.x), tf32_hi(im.y), tf32_hi(im.z), tf32_hi(im.w));
-                            const float4 rel = make_float4(re.x - reh.x, re.y - reh.y, re.z - reh.z, re.w - reh.w);
-                            const float4 iml = make_float4(im.x - imh.x, im.y - imh.y, im.z - imh.z, im.w - imh.w);
-                            unsigned char* unit = sm + (size_t)(slot * CHU + hsel * 4 + uu) * UNIT_BYTES;
-                            *reinterpret_cast<float4*>(unit + r * 16) = reh;
-                            *reinterpret_cast<float4*>(unit + (ROWS + r) * 16) = imh;
-                            *reinterpret_cast<float4*>(unit + OFF_LO + r * 16) = rel;
-                            *reinterpret_cast<float4*>(unit + OFF_LO + (ROWS + r) * 16) = iml;
+                        for (int i = 0; i < 4; ++i) {
+                            const float4 v = q[pi][i];                  // (re, im) of samples 2 (4i + piece), +1
+                            if (ci >= HALO_CH && hfirst >= 0 && rowok) {
+                                const int g = ms - HALF + ci * CHS + 2 * (4 * i + piece) - hfirst;
+                                float2* hrow = hnext + (size_t)row * (HALF - 1);
+                                if (g >= 0 && g < HALF - 1) hrow[g] = make_float2(v.x, v.y);
+                                if (g + 1 >= 0 && g + 1 < HALF - 1) hrow[g + 1] = make_float2(v.z, v.w);
+                            }
+                            const float rx = __shfl_xor_sync(0xffffffffu, odd ? v.x : v.y, 8);
+                            const float ry = __shfl_xor_sync(0xffffffffu, odd ? v.z : v.w, 8);
+                            const float4 w = odd ? make_float4(rx, ry, v.y, v.w) : make_float4(v.x, v.z, rx, ry);   // im[4] : re[4]
+                            const float4 wh = make_float4(tf32_hi(w.x), tf32_hi(w.y), tf32_hi(w.z), tf32_hi(w.w));
+                            const float4 wl = make_float4(w.x - wh.x, w.y - wh.y, w.z - wh.z, w.w - wh.w);
+                            const uint32_t addr = sbase + (uint32_t)(slot * CHU + 2 * i + (piece >> 1)) * UNIT_BYTES +
+                                                  (uint32_t)((odd ? ROWS : 0) + r) * 16;
+                            sts128(addr, wh);
+                            sts128(addr + OFF_LO, wl);
                         }
                         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
                         bar_arrive(full(slot));
+                        { TC_T0 issue(ci + PREFETCH, q[pi]); if (tid == 0) { TC_ACC(7) } }
                     }
                 }
             }
         } else
-        if (warp == 12) {
+        if (warp == LOADER_WARPS + EPI_WARPS) {
             // ===== MMA issuer (one thread) =====
             if (lane == 0) {
                 const uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(NR >> 3) << 17) | ((uint32_t)(MOUT >> 4) << 24);
                 const uint32_t d = tmem + COL_D;
                 for (int j = 0; j < J; ++j) {
                     const int cn = cbase + 2 * j + WIN_CH - 1;          // newest chunk of this tile's window
-                    bar_wait(full(cn % RING_CH), (uint32_t)((cn / RING_CH) & 1));
+                    { TC_T0 bar_wait(full(cn % RING_CH), (uint32_t)((cn / RING_CH) & 1)); TC_ACC(0) }
                     const int t = tbase + j;
-                    if (t > 0) bar_wait(tempty, (uint32_t)((t - 1) & 1));   // the previous tile's accumulator has been read
+                    { TC_T0 if (t > 0) bar_wait(tempty, (uint32_t)((t - 1) & 1)); TC_ACC(1) }   // the previous tile's accumulator has been read
                     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
                     const int wu0 = ((cbase + 2 * j) % RING_CH) * CHU;  // ring unit of the window's first unit
+                    TC_T0
 #pragma unroll 2
                     for (int ks = 0; ks < KSTEPS; ++ks) {
                         int ru = wu0 + 2 * ks;
@@ -290,42 +330,52 @@ __global__ void __launch_bounds__(THREADS, 1) spiir_up2_tc_kernel(const UpTcArgs
                     umma_commit(empty((cbase + 2 * j) % RING_CH));     // the window's two oldest chunks are free once these MMAs are done
                     umma_commit(empty((cbase + 2 * j + 1) % RING_CH));
                     umma_commit(tfull);
+                    TC_ACC(4)
                 }
                 for (int i = 0; i < HALO_CH; ++i) umma_commit(empty((cbase + 2 * J + i) % RING_CH));
             }
             __syncwarp();
         } else {
-            // ===== epilogue, 256 threads: TMEM lane = output sample, columns = real rows.  Warp group `half` takes the
-            // complex rows [32 half, 32 half + 32): re in columns 32 half.., im in columns 64 + 32 half.. =====
-            const int ew = warp & 3, half = (warp - 4) >> 2;
+            // ===== epilogue, 128 threads: TMEM lane = output sample, columns = real rows (re of row i in column i, im in
+            // column 64 + i), drained 16 rows at a time =====
+            const int ew = warp & 3;
             const int tl = ew * 32 + lane;                              // output index within the tile
-            const uint32_t taddr = tmem + ((uint32_t)(ew * 32) << 16) + COL_D + (uint32_t)(32 * half);
+            const uint32_t taddr = tmem + ((uint32_t)(ew * 32) << 16) + COL_D;
             for (int j = 0; j < J; ++j) {
                 const int t = tbase + j;
                 const int m0 = ms + j * TIN;
                 const bool tok = tl < 2 * min(TIN, a.n_in - m0);
-                float2* obase = a.out + (size_t)(row0 + 32 * half) * 2 * a.n_in + 2 * m0 + tl;
-                bar_wait(tfull, (uint32_t)(t & 1));
+                float2* obase = a.out + (size_t)row0 * 2 * a.n_in + 2 * m0 + tl;
+                { TC_T0 bar_wait(tfull, (uint32_t)(t & 1)); if (tid == LOADER_WARPS * 32) { TC_ACC(2) } }
                 asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-                uint32_t vre[32], vim[32];
-                tmem_ld32(taddr, vre);
-                tmem_ld32(taddr + ROWS, vim);
-                asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-                asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
-                bar_arrive(tempty);                                     // the accumulator may be overwritten
-                // accumulate = a vector reduction performed by the L2 (one addend per element and call: deterministic); no
-                // read-modify-write round trip through this thread's registers
-                if (a.accumulate) {
+                // drain 32 rows at a time (64 registers); the accumulator is released right after the second drain, so only
+                // the first half's stores sit between the end of this tile's MMAs and the start of the next tile's
 #pragma unroll
-                    for (int i = 0; i < 32; ++i)
-                        if (tok && row0 + 32 * half + i < a.rows)
-                            asm volatile("red.global.add.v2.f32 [%0], {%1, %2};" ::"l"(obase + (size_t)i * 2 * a.n_in),
-                                         "f"(__uint_as_float(vre[i])), "f"(__uint_as_float(vim[i])) : "memory");
-                } else {
+                for (int hh = 0; hh < 2; ++hh) {
+                    uint32_t vre[32], vim[32];
+                    tmem_ld32(taddr + 32 * hh, vre);
+                    tmem_ld32(taddr + ROWS + 32 * hh, vim);
+                    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+                    if (hh == 1) {
+                        asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+                        bar_arrive(tempty);                             // the accumulator may be overwritten
+                    }
+                    // accumulate = a vector reduction performed by the L2 (one addend per element and call: deterministic);
+                    // no read-modify-write round trip through this thread's registers
+                    float2* ob = obase + (size_t)(32 * hh) * 2 * a.n_in;
+                    const int rbase = row0 + 32 * hh;
+                    if (a.accumulate) {
 #pragma unroll
-                    for (int i = 0; i < 32; ++i)
-                        if (tok && row0 + 32 * half + i < a.rows)
-                            obase[(size_t)i * 2 * a.n_in] = make_float2(__uint_as_float(vre[i]), __uint_as_float(vim[i]));
+                        for (int i = 0; i < 32; ++i)
+                            if (tok && rbase + i < a.rows)
+                                asm volatile("red.global.add.v2.f32 [%0], {%1, %2};" ::"l"(ob + (size_t)i * 2 * a.n_in),
+                                             "f"(__uint_as_float(vre[i])), "f"(__uint_as_float(vim[i])) : "memory");
+                    } else {
+#pragma unroll
+                        for (int i = 0; i < 32; ++i)
+                            if (tok && rbase + i < a.rows)
+                                ob[(size_t)i * 2 * a.n_in] = make_float2(__uint_as_float(vre[i]), __uint_as_float(vim[i]));
+                    }
                 }
             }
         }
@@ -335,7 +385,7 @@ __global__ void __launch_bounds__(THREADS, 1) spiir_up2_tc_kernel(const UpTcArgs
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     const bool last = last_cta_arrives(a.phase, gridDim.x);           // __syncthreads inside
     if (last) a.phase[0] = ph ^ 1;
-    if (warp == 12) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"(TMEM_COLS));
+    if (warp == LOADER_WARPS + EPI_WARPS) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"(TMEM_COLS));
 }
 
 }  // namespace tc
