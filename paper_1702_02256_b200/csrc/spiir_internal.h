@@ -114,7 +114,6 @@ struct spiir_resamp {
     int direction = 0, N = 0, rows = 0, max_block = 0;
     int H = 0;                        // history samples per row
     float* d_taps = nullptr;
-    float* d_bmat = nullptr;          // up stage, 192 taps: Toeplitz operand of the tensor-core FIR (hi, lo parts)
     int flags = 0;                    // spiir_resamp_opts.flags
     void* d_hist[2] = {nullptr, nullptr};
     int* d_phase = nullptr;           // {phase, arrivals}

@@ -23,7 +23,6 @@ size_t resamp_layout(spiir_resamp* r, Arena* a)
     const size_t start = a->used;
     r->d_phase = a->take_n<int>(64);
     r->d_taps = a->take_n<float>((size_t)r->N);
-    r->d_bmat = (r->direction == SPIIR_UP2 && r->N == 2 * tc::HALF) ? a->take_n<float>(tc::TMAT_FLOATS) : nullptr;
     r->d_hist[0] = a->take(hist_bytes(r));
     r->d_hist[1] = a->take(hist_bytes(r));
     a->used = (a->used + 255) & ~(size_t)255;
@@ -39,28 +38,6 @@ static void resamp_shape(spiir_resamp* r, int direction, int n_taps, int n_rows,
 {
     r->direction = direction; r->N = n_taps; r->rows = n_rows; r->max_block = max_block;
     r->H = direction == SPIIR_DOWN2 ? n_taps - 1 : n_taps / 2 - 1;
-}
-
-// Toeplitz operand of the tensor-core up FIR (spiir_resample_tc.cuh): T[t = 2m'+p][k] = 2 h[2 (96 + m' - k) + p] for
-// 1 <= k - m' <= 96, row-major [128][160], split into a TF32-exact high part (round to nearest, ties away) and the
-// float32 remainder; the kernel copies it into tensor memory once per CTA.
-static void build_up_tc_operand(const std::vector<float>& taps, std::vector<float>* tm)
-{
-    const size_t part = (size_t)tc::MOUT * tc::KWIN;
-    tm->assign(2 * part, 0.f);
-    for (int t = 0; t < tc::MOUT; ++t)
-        for (int k = 0; k < tc::KWIN; ++k) {
-            const int mp = t >> 1, p = t & 1, dk = k - mp;
-            if (dk < 1 || dk > tc::HALF) continue;
-            const float v = 2.f * taps[2 * (tc::HALF + mp - k) + p];
-            uint32_t b;
-            memcpy(&b, &v, 4);
-            b = (b + 0x1000u) & 0xffffe000u;
-            float hi;
-            memcpy(&hi, &b, 4);
-            (*tm)[(size_t)t * tc::KWIN + k] = hi;
-            (*tm)[part + (size_t)t * tc::KWIN + k] = v - hi;
-        }
 }
 
 spiir_status resamp_create_in(spiir_resamp_t** out, int direction, int n_taps, double kaiser_beta, double cutoff, int n_rows,
@@ -83,11 +60,6 @@ spiir_status resamp_create_in(spiir_resamp_t** out, int direction, int n_taps, d
     resamp_layout(r, &r->arena);
     cudaError_t e = cudaMemset(r->d_phase, 0, 64 * sizeof(int));
     if (e == cudaSuccess) e = cudaMemcpy(r->d_taps, r->taps.data(), n_taps * sizeof(float), cudaMemcpyHostToDevice);
-    if (e == cudaSuccess && r->d_bmat) {
-        std::vector<float> bm;
-        build_up_tc_operand(r->taps, &bm);
-        e = cudaMemcpy(r->d_bmat, bm.data(), bm.size() * sizeof(float), cudaMemcpyHostToDevice);
-    }
     if (e == cudaSuccess) e = cudaMemset(r->d_hist[0], 0, hist_bytes(r));
     if (e == cudaSuccess) e = cudaMemset(r->d_hist[1], 0, hist_bytes(r));
     if (e != cudaSuccess) { rc = cuda_fail(e, "spiir_resamp_create initialisation"); delete r; return rc; }
@@ -271,9 +243,9 @@ spiir_status spiir_resample_up(spiir_resamp_t* r, const spiir_c64* in, int n_in,
     }
     // 192 taps on the tensor cores (tcgen05 kind::tf32, three-pass split): FP32-bound on the CUDA cores, HBM-bound here.
     // Needs enough work to fill the persistent CTAs; small calls keep the register-blocked kernel.
-    if (r->N == 2 * tc::HALF && r->d_bmat && !(r->flags & 1) && (long long)r->rows * n_in >= 64LL * 1024) {
+    if (r->N == 2 * tc::HALF && !(r->flags & 1) && (long long)r->rows * n_in >= 64LL * 1024) {
         tc::UpTcArgs t;
-        t.in = u.in; t.out = u.out; t.hbuf[0] = u.hbuf[0]; t.hbuf[1] = u.hbuf[1]; t.phase = u.phase; t.tmat = r->d_bmat;
+        t.in = u.in; t.out = u.out; t.hbuf[0] = u.hbuf[0]; t.hbuf[1] = u.hbuf[1]; t.phase = u.phase; t.taps = r->d_taps;
         t.rows = r->rows; t.n_in = n_in; t.accumulate = accumulate;
         t.tiles_per_row = (n_in + tc::TIN - 1) / tc::TIN;
         t.nstrips = (r->rows + tc::ROWS - 1) / tc::ROWS;

@@ -2,29 +2,29 @@
 // (row a10 of SURVEY.md section 8; Eq. 9).
 //
 // The polyphase FIR  w[2m+p] = 2 sum_{q<96} h[2q+p] v[m-q]  of a strip of 64 complex rows is a dense contraction
-// with a banded Toeplitz matrix, one tile = 64 input positions -> 128 outputs:
+// with a banded Toeplitz matrix; a strip is 48 complex rows, one tile = 64 input positions -> 128 outputs:
 //     D[t, row'] = sum_k T[t, k] * X[row', k]
 //   T: 128 outputs of the tile x a window of K = 160 input samples (96 before the tile + its 64 inputs),
 //      T[2m'+p, k] = 2 h[2 (96 + m' - k) + p] for 1 <= k - m' <= 96, zero elsewhere (60 % dense).  It is the same for
 //      every tile, so it lives in TENSOR MEMORY for the whole kernel (the A operand of tcgen05.mma may come from TMEM);
-//   X: 128 real rows (re of the 64 rows, then im) x the window, the DATA, in shared memory (B operand, K-major);
-//   D: 128 lanes (outputs) x 128 columns (real rows) of float32 in TMEM.
-// tcgen05.mma kind::tf32 (M = 128, N = 128, K = 8 per instruction: measured 67 cycles, i.e. the nominal TF32 rate;
-// N <= 64 costs the same 55 cycles per instruction, so narrow tiles waste the pipe).  One TF32 pass has 2^-11
+//   X: 96 real rows (re of the 48 rows, then im) x the window, the DATA, in shared memory (B operand, K-major);
+//   D: 128 lanes (outputs) x 96 columns (real rows) of float32 in TMEM, double-buffered (320 + 2 x 96 = all 512 columns).
+// tcgen05.mma kind::tf32 (M = 128, N = 96, K = 8 per instruction; measured on this B200: 55 cycles per instruction
+// up to N = 64, 67 at N = 128 = the nominal TF32 rate, so narrow tiles waste the pipe).  One TF32 pass has 2^-11
 // input precision, far outside the 1e-5 tolerance: every operand is split into a TF32-exact high part and the
 // float32 remainder and three passes are accumulated, T_hi X_hi + T_lo X_hi + T_hi X_lo (the dropped T_lo X_lo
 // term is 2^-22 relative).
 //
 // The data operand uses the canonical K-major, non-swizzled layout: 16-byte "units" of 4 consecutive samples,
-// unit u of real row r at u * 2048 + r * 16.  It is a RING of 48 units (6 chunks of 32 samples): a tile's window
-// is 5 consecutive chunks, every tile advances it by two, so each input sample is written to shared memory once
-// and read by 2.5 tiles; a K = 8 instruction takes two adjacent units and never straddles the ring's end.
+// unit u of real row r at u * 1536 + r * 16.  It is a RING of 56 units (7 chunks of 32 samples): a tile's window
+// is 5 consecutive chunks, every tile advances it by two and two chunks are free for the loader to run a whole tile
+// ahead; each input sample is written to shared memory once and read by 2.5 tiles; a K = 8 instruction takes two adjacent units and never straddles the ring's end.
 //
-// Roles (416 threads): warps 0-7 load + split + store the data chunks (global loads prefetched four chunks deep in
-// registers: 64 KB in flight per SM), warp 12 issues the MMAs (one thread) and owns TMEM, warps 8-11 drain the accumulator (tcgen05.ld):
+// Roles (352 threads): warps 0-5 load + split + store the data chunks (8 rows per warp, global loads prefetched four
+// chunks deep in registers), warp 10 issues the MMAs (one thread) and owns TMEM, warps 6-9 drain the accumulator (tcgen05.ld):
 // a lane is an output sample, so a warp writes 256 contiguous bytes of one row per store -- no transposition; with
-// accumulate the store is a vector reduction (red.global.add.v2.f32) done by the L2.  mbarriers: full[6] /
-// empty[6] per ring chunk, tfull / tempty for the accumulator.  CTAs are persistent over (strip, time segment) units.
+// accumulate the store is a vector reduction (red.global.add.v2.f32) done by the L2.  mbarriers: full[7] /
+// empty[7] per ring chunk, tfull[2] / tempty[2] for the accumulator buffers.  CTAs are persistent over (strip, time segment) units.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -33,16 +33,8 @@
 
 namespace spiir {
 namespace tc {
-#ifdef SPIIR_TC_DEBUG
-__device__ long long g_dbg[16];
-#define TC_T0 const long long t0__ = clock64();
-#define TC_ACC(i) if (blockIdx.x == 0) atomicAdd((unsigned long long*)&g_dbg[i], (unsigned long long)(clock64() - t0__));
-#else
-#define TC_T0
-#define TC_ACC(i)
-#endif
 
-constexpr int ROWS = 64;                       // complex rows per strip
+constexpr int ROWS = 48;                       // complex rows per strip (96 real rows: the ring then has a whole tile of slack)
 constexpr int NR = 2 * ROWS;                   // real rows = UMMA N
 constexpr int TIN = 64;                        // input samples per tile
 constexpr int MOUT = 2 * TIN;                  // outputs per tile = UMMA M
@@ -53,29 +45,28 @@ constexpr int CHS = 32;                        // samples per chunk
 constexpr int CHU = CHS / 4;                   // units per chunk
 constexpr int WIN_CH = KWIN / CHS;             // 5 chunks per window
 constexpr int HALO_CH = HALF / CHS;            // 3 chunks in front of the first tile of a unit
-constexpr int RING_CH = WIN_CH + 1;            // one chunk of prefetch space
-constexpr int RING_UNITS = RING_CH * CHU;      // 48 (even)
+constexpr int RING_CH = WIN_CH + 2;            // a whole tile (two chunks) of prefetch space
+constexpr int RING_UNITS = RING_CH * CHU;      // 56 (even)
 constexpr int UNIT_BYTES = NR * 16;
 constexpr int PART_BYTES = RING_UNITS * UNIT_BYTES;
 constexpr int OFF_LO = PART_BYTES;
 constexpr int OFF_BAR = 2 * PART_BYTES;
-constexpr int NBAR = 2 * RING_CH + 2;
+constexpr int NBAR = 2 * RING_CH + 4;
 constexpr int OFF_TPTR = OFF_BAR + NBAR * 8;
 constexpr int SMEM_BYTES = OFF_TPTR + 16;
-constexpr int LOADER_WARPS = 8;
+constexpr int LOADER_WARPS = ROWS / 8;         // a loader warp owns 8 rows
 constexpr int EPI_WARPS = 4;
 constexpr int THREADS = (LOADER_WARPS + EPI_WARPS + 1) * 32;   // loader warps, epilogue warps, 1 MMA warp (416: 128 registers each)
 constexpr int PREFETCH = 4;                    // chunks of global loads in flight per loader thread (64 KB per CTA)
 constexpr int TMEM_COLS = 512;
-constexpr int COL_THI = 0, COL_TLO = KWIN, COL_D = 384;
-constexpr int TMAT_FLOATS = 2 * MOUT * KWIN;   // T_hi then T_lo, [128][160] each
+constexpr int COL_THI = 0, COL_TLO = KWIN, COL_D = 2 * KWIN;   // two accumulator buffers of NR columns at COL_D: 320 + 2 * 96 = 512
 
 struct UpTcArgs {
     const float2* in;        // [rows][n_in]
     float2*       out;       // [rows][2 n_in]
     float2*       hbuf[2];   // [rows][95] ping-pong history
     int*          phase;
-    const float*  tmat;      // DEVICE: T_hi [128][160] then T_lo [128][160]
+    const float*  taps;      // DEVICE: the 192 taps h[j]
     int rows, n_in, accumulate;
     int nstrips, nsegs, seg_tiles, tiles_per_row;
     int in16;                // rows of `in` are 16-byte aligned
@@ -172,7 +163,8 @@ __global__ void __launch_bounds__(THREADS, 1) spiir_up2_tc_kernel(const UpTcArgs
     const uint32_t bar0 = sbase + OFF_BAR;
     auto full = [&](int i) { return bar0 + 8u * (uint32_t)i; };
     auto empty = [&](int i) { return bar0 + 8u * (uint32_t)(RING_CH + i); };
-    const uint32_t tfull = bar0 + 8u * (uint32_t)(2 * RING_CH), tempty = tfull + 8u;
+    auto tfull = [&](int i) { return bar0 + 8u * (uint32_t)(2 * RING_CH + i); };
+    auto tempty = [&](int i) { return bar0 + 8u * (uint32_t)(2 * RING_CH + 2 + i); };
     uint32_t* tptr = reinterpret_cast<uint32_t*>(sm + OFF_TPTR);
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int ph = phase_read(a.phase);
@@ -181,9 +173,8 @@ __global__ void __launch_bounds__(THREADS, 1) spiir_up2_tc_kernel(const UpTcArgs
 
     // ---- one-time setup: barriers, tensor memory, the Toeplitz operand into TMEM --------------------------
     if (tid == 0) {
-        for (int i = 0; i < RING_CH; ++i) { bar_init(full(i), LOADER_WARPS * 32); bar_init(empty(i), 1); }
-        bar_init(tfull, 1);
-        bar_init(tempty, EPI_WARPS * 32);
+        for (int i = 0; i < RING_CH; ++i) { bar_init(full(i), LOADER_WARPS); bar_init(empty(i), 1); }
+        for (int i = 0; i < 2; ++i) { bar_init(tfull(i), 1); bar_init(tempty(i), EPI_WARPS); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     if (warp == LOADER_WARPS + EPI_WARPS) {
@@ -197,14 +188,21 @@ __global__ void __launch_bounds__(THREADS, 1) spiir_up2_tc_kernel(const UpTcArgs
     if (warp >= LOADER_WARPS && warp < LOADER_WARPS + 4) {             // lane t of TMEM = output t of a tile
         const int t = (warp & 3) * 32 + lane;
         const uint32_t lane_addr = tmem + ((uint32_t)((warp & 3) * 32) << 16);
-        for (int part = 0; part < 2; ++part) {
-            const float* src = a.tmat + ((size_t)part * MOUT + t) * KWIN;
-            for (int c0 = 0; c0 < KWIN; c0 += 32) {
-                uint32_t v[32];
+        // T[t = 2m'+p][k] = 2 h[2 (96 + m' - k) + p] for 1 <= k - m' <= 96, split into a TF32-exact high part and the
+        // float32 remainder, computed from the 192 taps (L1-resident) straight into this thread's TMEM lane
+        const int mp = t >> 1, pp = t & 1;
+        for (int c0 = 0; c0 < KWIN; c0 += 32) {
+            uint32_t vh[32], vl[32];
 #pragma unroll
-                for (int i = 0; i < 32; ++i) v[i] = __float_as_uint(src[c0 + i]);
-                tmem_st32(lane_addr + (uint32_t)(part ? COL_TLO : COL_THI) + (uint32_t)c0, v);
+            for (int i = 0; i < 32; ++i) {
+                const int dk = c0 + i - mp;
+                const float v = (dk >= 1 && dk <= HALF) ? 2.f * __ldg(a.taps + 2 * (HALF - dk) + pp) : 0.f;
+                const float h = tf32_hi(v);
+                vh[i] = __float_as_uint(h);
+                vl[i] = __float_as_uint(v - h);
             }
+            tmem_st32(lane_addr + COL_THI + (uint32_t)c0, vh);
+            tmem_st32(lane_addr + COL_TLO + (uint32_t)c0, vl);
         }
         asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
     }
@@ -276,7 +274,7 @@ __global__ void __launch_bounds__(THREADS, 1) spiir_up2_tc_kernel(const UpTcArgs
                     const int ci = c0 + pi;
                     if (ci < nch) {                                      // uniform over the CTA's loader threads
                         const int c = cbase + ci, slot = c % RING_CH, fill = c / RING_CH;
-                        { TC_T0 if (fill > 0) bar_wait(empty(slot), (uint32_t)((fill - 1) & 1)); if (tid == 0) { TC_ACC(3) } }
+                        if (fill > 0) bar_wait(empty(slot), (uint32_t)((fill - 1) & 1));
 #pragma unroll
                         for (int i = 0; i < 4; ++i) {
                             const float4 v = q[pi][i];                  // (re, im) of samples 2 (4i + piece), +1
@@ -297,8 +295,9 @@ __global__ void __launch_bounds__(THREADS, 1) spiir_up2_tc_kernel(const UpTcArgs
                             sts128(addr + OFF_LO, wl);
                         }
                         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-                        bar_arrive(full(slot));
-                        { TC_T0 issue(ci + PREFETCH, q[pi]); if (tid == 0) { TC_ACC(7) } }
+                        __syncwarp();
+                        if (lane == 0) bar_arrive(full(slot));          // one arrival per warp
+                        issue(ci + PREFETCH, q[pi]);
                     }
                 }
             }
@@ -307,15 +306,14 @@ __global__ void __launch_bounds__(THREADS, 1) spiir_up2_tc_kernel(const UpTcArgs
             // ===== MMA issuer (one thread) =====
             if (lane == 0) {
                 const uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(NR >> 3) << 17) | ((uint32_t)(MOUT >> 4) << 24);
-                const uint32_t d = tmem + COL_D;
                 for (int j = 0; j < J; ++j) {
                     const int cn = cbase + 2 * j + WIN_CH - 1;          // newest chunk of this tile's window
-                    { TC_T0 bar_wait(full(cn % RING_CH), (uint32_t)((cn / RING_CH) & 1)); TC_ACC(0) }
-                    const int t = tbase + j;
-                    { TC_T0 if (t > 0) bar_wait(tempty, (uint32_t)((t - 1) & 1)); TC_ACC(1) }   // the previous tile's accumulator has been read
+                    bar_wait(full(cn % RING_CH), (uint32_t)((cn / RING_CH) & 1));
+                    const int t = tbase + j, buf = t & 1, use = t >> 1;
+                    if (use > 0) bar_wait(tempty(buf), (uint32_t)((use - 1) & 1));   // this buffer's previous tile has been drained
+                    const uint32_t d = tmem + COL_D + (uint32_t)(buf * NR);
                     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
                     const int wu0 = ((cbase + 2 * j) % RING_CH) * CHU;  // ring unit of the window's first unit
-                    TC_T0
 #pragma unroll 2
                     for (int ks = 0; ks < KSTEPS; ++ks) {
                         int ru = wu0 + 2 * ks;
@@ -329,52 +327,53 @@ __global__ void __launch_bounds__(THREADS, 1) spiir_up2_tc_kernel(const UpTcArgs
                     }
                     umma_commit(empty((cbase + 2 * j) % RING_CH));     // the window's two oldest chunks are free once these MMAs are done
                     umma_commit(empty((cbase + 2 * j + 1) % RING_CH));
-                    umma_commit(tfull);
-                    TC_ACC(4)
+                    umma_commit(tfull(buf));
                 }
                 for (int i = 0; i < HALO_CH; ++i) umma_commit(empty((cbase + 2 * J + i) % RING_CH));
             }
             __syncwarp();
         } else {
             // ===== epilogue, 128 threads: TMEM lane = output sample, columns = real rows (re of row i in column i, im in
-            // column 64 + i), drained 16 rows at a time =====
+            // column ROWS + i).  The thread drains its whole accumulator row into registers, releases the buffer at once
+            // (the next-but-one tile's MMAs may overwrite it) and then stores: a warp writes 256 contiguous bytes of one
+            // output row per instruction, no transposition. =====
             const int ew = warp & 3;
             const int tl = ew * 32 + lane;                              // output index within the tile
-            const uint32_t taddr = tmem + ((uint32_t)(ew * 32) << 16) + COL_D;
             for (int j = 0; j < J; ++j) {
-                const int t = tbase + j;
+                const int t = tbase + j, buf = t & 1, use = t >> 1;
                 const int m0 = ms + j * TIN;
                 const bool tok = tl < 2 * min(TIN, a.n_in - m0);
                 float2* obase = a.out + (size_t)row0 * 2 * a.n_in + 2 * m0 + tl;
-                { TC_T0 bar_wait(tfull, (uint32_t)(t & 1)); if (tid == LOADER_WARPS * 32) { TC_ACC(2) } }
+                const uint32_t taddr = tmem + ((uint32_t)(ew * 32) << 16) + COL_D + (uint32_t)(buf * NR);
+                bar_wait(tfull(buf), (uint32_t)(use & 1));
                 asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-                // drain 32 rows at a time (64 registers); the accumulator is released right after the second drain, so only
-                // the first half's stores sit between the end of this tile's MMAs and the start of the next tile's
+                uint32_t vre[ROWS / 16][16], vim[ROWS / 16][16];
 #pragma unroll
-                for (int hh = 0; hh < 2; ++hh) {
-                    uint32_t vre[32], vim[32];
-                    tmem_ld32(taddr + 32 * hh, vre);
-                    tmem_ld32(taddr + ROWS + 32 * hh, vim);
-                    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-                    if (hh == 1) {
-                        asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
-                        bar_arrive(tempty);                             // the accumulator may be overwritten
-                    }
-                    // accumulate = a vector reduction performed by the L2 (one addend per element and call: deterministic);
-                    // no read-modify-write round trip through this thread's registers
-                    float2* ob = obase + (size_t)(32 * hh) * 2 * a.n_in;
-                    const int rbase = row0 + 32 * hh;
+                for (int hh = 0; hh < ROWS / 16; ++hh) {
+                    tmem_ld16(taddr + 16 * hh, vre[hh]);
+                    tmem_ld16(taddr + ROWS + 16 * hh, vim[hh]);
+                }
+                asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+                asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+                __syncwarp();
+                if (lane == 0) bar_arrive(tempty(buf));
+                // accumulate = a vector reduction performed by the L2 (one addend per element and call: deterministic);
+                // no read-modify-write round trip through this thread's registers
+#pragma unroll
+                for (int hh = 0; hh < ROWS / 16; ++hh) {
+                    float2* ob = obase + (size_t)(16 * hh) * 2 * a.n_in;
+                    const int rbase = row0 + 16 * hh;
                     if (a.accumulate) {
 #pragma unroll
-                        for (int i = 0; i < 32; ++i)
+                        for (int i = 0; i < 16; ++i)
                             if (tok && rbase + i < a.rows)
                                 asm volatile("red.global.add.v2.f32 [%0], {%1, %2};" ::"l"(ob + (size_t)i * 2 * a.n_in),
-                                             "f"(__uint_as_float(vre[i])), "f"(__uint_as_float(vim[i])) : "memory");
+                                             "f"(__uint_as_float(vre[hh][i])), "f"(__uint_as_float(vim[hh][i])) : "memory");
                     } else {
 #pragma unroll
-                        for (int i = 0; i < 32; ++i)
+                        for (int i = 0; i < 16; ++i)
                             if (tok && rbase + i < a.rows)
-                                ob[(size_t)i * 2 * a.n_in] = make_float2(__uint_as_float(vre[i]), __uint_as_float(vim[i]));
+                                ob[(size_t)i * 2 * a.n_in] = make_float2(__uint_as_float(vre[hh][i]), __uint_as_float(vim[hh][i]));
                     }
                 }
             }

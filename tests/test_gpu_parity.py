@@ -519,6 +519,29 @@ def test_resample_up_and_accumulate(sp, oracle_mod, rows, blocks):
     assert_parity(np.concatenate(zs, -1), np.concatenate(rs, -1), "up2")
 
 
+@pytest.mark.parametrize("rows,blocks,acc", [(130, (1024, 512, 576), True), (49, (2048, 1400), False), (700, (128, 160, 96), True)])
+def test_resample_up_tensor_core_path(sp, oracle_mod, rows, blocks, acc):
+    """The 192-tap up stage of a large call runs on the tensor cores (tcgen05 kind::tf32, three-pass split, PAPER.md:81-88):
+    streamed blocks (history carried through the loader), partial strips of rows, partial time tiles, with and without
+    accumulation, against the float64 oracle AND against the CUDA-core kernel (flags = 1)."""
+    import torch
+    rng = np.random.default_rng(rows)
+    tcr = sp.Resampler("up", rows, max_block=max(blocks))
+    ccr = sp.Resampler("up", rows, max_block=max(blocks), flags=1)
+    orc = oracle_mod.ResampOracle("up", rows)
+    for n in blocks:
+        assert rows * n >= 65536                                        # the size from which spiir_resample_up goes to the tensor cores
+        v = (rng.standard_normal((rows, n)) + 1j * rng.standard_normal((rows, n))).astype(np.complex64)
+        base = (rng.standard_normal((rows, 2 * n)) + 1j * rng.standard_normal((rows, 2 * n))).astype(np.complex64)
+        o1 = torch.from_numpy(base.copy()).cuda()
+        o2 = torch.from_numpy(base.copy()).cuda()
+        tcr.up(torch.from_numpy(v).cuda(), o1, accumulate=acc)
+        ccr.up(torch.from_numpy(v).cuda(), o2, accumulate=acc)
+        ref = orc.up(v) + (base.astype(np.complex128) if acc else 0.0)
+        assert_parity(o1.cpu().numpy(), ref, f"tensor-core up rows={rows} n={n}")
+        assert_parity(o2.cpu().numpy(), ref, f"cuda-core up rows={rows} n={n}")
+
+
 @pytest.mark.parametrize("n_taps", [32, 64, 192, 384])
 def test_resamplers_other_tap_counts_and_odd_shapes(sp, oracle_mod, n_taps):
     """32, 192 and (down only) 384 taps take the register-blocked kernels (taps in the kernel parameters), 64 and
