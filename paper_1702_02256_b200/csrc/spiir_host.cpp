@@ -41,10 +41,20 @@ bool choose_lane_mapping(int L, int T, int* F, int* LPT, int* NP)
     // (two templates per warp).  The 16 outputs of a batch then cost a 16-lane butterfly for TWO templates,
     // i.e. half the shuffle / select work per update of the one-warp-per-template mapping.
     if (L >= 32 && L <= 128 && T >= lpt16_min_templates()) { *LPT = 16; *F = (L + 15) / 16; return true; }
-    if (L <= 4) { *LPT = 1; *F = L; return true; }
-    if (L <= 8) { *LPT = 2; *F = (L + 1) / 2; return true; }
-    if (L <= 16) { *LPT = 4; *F = (L + 3) / 4; return true; }
-    if (L < 32) { *LPT = 8; *F = (L + 7) / 8; return true; }
+    if (L < 32) {
+        if (L <= 4) { *LPT = 1; *F = L; }
+        else if (L <= 8) { *LPT = 2; *F = (L + 1) / 2; }
+        else if (L <= 16) { *LPT = 4; *F = (L + 3) / 4; }
+        else { *LPT = 8; *F = (L + 7) / 8; }
+        // A mid-sized bank of very short templates gives too few warp tasks (= CTAs of the in-CTA time scan) to cover the
+        // SMs: 1024 templates x 8 filters at 2 lanes each are 64 tasks on 148 SMs.  Twice the lanes per template doubles
+        // the tasks; the extra butterfly stage costs less than the idle SMs (configs[3] base rate: 69 -> 40 us).
+        while (T >= 512 && *LPT < 8 && *F >= 4 && (long)((T * *LPT + 31) / 32) * 4 < 3L * 148) {
+            *LPT *= 2;
+            *F = (L + *LPT - 1) / *LPT;
+        }
+        return true;
+    }
     *LPT = 32;
     if (L <= 512) {
         const int need = (L + 31) / 32;

@@ -375,11 +375,12 @@ constexpr int kDownSegMax = 128 * kDownR;              // outputs per row segmen
 template <int N>
 struct DownTaps { float h[N]; };
 
-template <int N>
+template <int N, int R = kDownR>
 __device__ __forceinline__ void down2_units(const float* __restrict__ w, int n_out, float* __restrict__ out_s,
                                             const DownTaps<N>& taps, int first_unit, int unit_stride)
 {
-    constexpr int R = kDownR, NIN = N + 2 * R - 2, NLD = (NIN + 3) / 4;
+    static_assert(R % 2 == 0, "a unit starts at word 2 R unit: 16-byte aligned only for even R");
+    constexpr int NIN = N + 2 * R - 2, NLD = (NIN + 3) / 4;
     for (int unit = first_unit; unit * R < n_out; unit += unit_stride) {
         const float4* wp = reinterpret_cast<const float4*>(w + 2 * unit * R);
         float acc[R];
@@ -469,6 +470,13 @@ struct DownChainArgs {
     int n, nstages;
 };
 
+__device__ __forceinline__ int ph_of(const int (&ph)[15], int k)
+{
+    int v = 0;
+#pragma unroll
+    for (int i = 0; i < 15; ++i) v = (i == k) ? ph[i] : v;
+    return v;
+}
 constexpr int kChainPad = 32;        // zeroed words after a buffer (the 16-byte loads of the last unit over-read)
 __host__ __device__ inline int down_chain_buf_len(int N, int n_in) { return (N - 1 + n_in + kChainPad + 3) & ~3; }
 
@@ -479,30 +487,49 @@ __global__ void __launch_bounds__(512) spiir_down_chain_kernel(const DownChainAr
     extern __shared__ __align__(16) float smd[];
     const int s = blockIdx.x;
     float* w = smd;                                                     // [history H | data n_in | pad]
-    {   // stage-0 input: history of stage 0 and the caller's block
-        const float* x = a.x + (size_t)s * a.n;
-        const float* h0 = a.hbuf[0][phase_read(a.phase[0])] + (size_t)s * H;
-        const int len = down_chain_buf_len(N, a.n);
-        for (int i = threadIdx.x; i < len; i += blockDim.x)
-            w[i] = i < H ? h0[i] : (i < H + a.n ? x[i - H] : 0.f);
+    int ph[kMaxStages];
+    {   // Every stage's history and zero pad, and the caller's block, up front.  All phase words are read first, then all
+        // history words of this thread are fetched before any of them is stored: two DRAM round trips in total instead
+        // of two per stage.
+#pragma unroll
+        for (int k = 0; k < kMaxStages; ++k) ph[k] = k < a.nstages ? phase_read(a.phase[k]) : 0;
+        const float* __restrict__ xr = a.x + (size_t)s * a.n;
+        float hv[kMaxStages];
+#pragma unroll
+        for (int k = 0; k < kMaxStages; ++k)
+            hv[k] = (k < a.nstages && (int)threadIdx.x < H) ? a.hbuf[k][ph[k]][(size_t)s * H + threadIdx.x] : 0.f;
+        static_assert(H <= 512, "one history word per thread and stage");
+        float* wk = smd;
+        int n_k = a.n;
+#pragma unroll
+        for (int k = 0; k < kMaxStages; ++k) {
+            if (k < a.nstages) {
+                const int len = down_chain_buf_len(N, n_k);
+                if ((int)threadIdx.x < H) wk[threadIdx.x] = hv[k];
+                for (int i = H + n_k + threadIdx.x; i < len; i += blockDim.x) wk[i] = 0.f;
+                if (k == 0) {
+                    float* wd = wk + H;
+#pragma unroll 8
+                    for (int i = threadIdx.x; i < n_k; i += blockDim.x) wd[i] = xr[i];
+                }
+                wk += len; n_k >>= 1;
+            }
+        }
     }
     int n_in = a.n;
     for (int k = 0; k < a.nstages; ++k) {
         const int n_out = n_in >> 1;
         float* wn = w + down_chain_buf_len(N, n_in);                    // buffer of the next stage
-        const int len_n = down_chain_buf_len(N, n_out);
-        if (k + 1 < a.nstages) {                                        // its history and zero pad
-            const float* hk = a.hbuf[k + 1][phase_read(a.phase[k + 1])] + (size_t)s * H;
-            for (int i = threadIdx.x; i < len_n; i += blockDim.x)
-                if (i < H || i >= H + n_out) wn[i] = i < H ? hk[i] : 0.f;
-        }
         __syncthreads();
-        down2_units<N>(w, n_out, wn + H, taps, threadIdx.x, blockDim.x);
+        // outputs per thread: as few as keep all threads busy (a thread's FIR is a serial chain of N R FMAs)
+        if (n_out > 4 * (int)blockDim.x) down2_units<N, kDownR>(w, n_out, wn + H, taps, threadIdx.x, blockDim.x);
+        else if (n_out > 2 * (int)blockDim.x) down2_units<N, 4>(w, n_out, wn + H, taps, threadIdx.x, blockDim.x);
+        else down2_units<N, 2>(w, n_out, wn + H, taps, threadIdx.x, blockDim.x);
         __syncthreads();
         float* o = a.xh[k] + (size_t)s * n_out;
         for (int i = threadIdx.x; i < n_out; i += blockDim.x) o[i] = wn[H + i];
         // carried history of stage k: the last H words of [history | data]
-        float* hn = a.hbuf[k][phase_read(a.phase[k]) ^ 1] + (size_t)s * H;
+        float* hn = a.hbuf[k][ph_of(ph, k) ^ 1] + (size_t)s * H;
         for (int i = threadIdx.x; i < H; i += blockDim.x) hn[i] = w[n_in + i];
         w = wn; n_in = n_out;
     }
