@@ -49,9 +49,9 @@ FP32_LANES_PER_SM = 128         # B200 SM: 4 sub-partitions x 32 FP32 lanes (gui
 HBM_FALLBACK_GBS = 7700.0       # B200_PROFILING.md nominal figure, used only when MEASURED_PEAKS.json is absent
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE spiir_filter_kernel launch, copied from the committed
 # `ncu --set full` captures named in TRAFFIC_SOURCE; per launch, like roofline.achieved.  Not measured by this run.
-NCU_DRAM_TRAFFIC = {"cfg1_many_filter_1024x256": 7.428352e6 + 0.137472e6,
-                    "cfg4_full_bank_2x16384x256": 235.036672e6 + 556.152064e6}
-TRAFFIC_SOURCE = ("constant from the ncu --set full capture in profiles/ (r1c_summary.md), not measured by this run; "
+NCU_DRAM_TRAFFIC = {"cfg1_many_filter_1024x256": 7.425536e6 + 0.019456e6,
+                    "cfg4_full_bank_2x16384x256": 235.016960e6 + 546.211072e6}
+TRAFFIC_SOURCE = ("constant from the ncu --set full capture in profiles/r2_summary.md, not measured by this run; "
                   "configs[1]: coefficients, delays and state once per block; the 33.5 MB SNR block is still in the "
                   "126 MB L2 when the kernel ends and is evicted by the flush outside the events")
 
