@@ -34,7 +34,10 @@
 namespace spiir {
 namespace tc {
 
-constexpr int ROWS = 48;                       // complex rows per strip (96 real rows: the ring then has a whole tile of slack)
+#ifndef SPIIR_TC_ROWS
+#define SPIIR_TC_ROWS 48
+#endif
+constexpr int ROWS = SPIIR_TC_ROWS;            // complex rows per strip: 48 (double-buffered accumulator; 327 us) or 64 (N = 128, single buffer; 375 us)
 constexpr int NR = 2 * ROWS;                   // real rows = UMMA N
 constexpr int TIN = 64;                        // input samples per tile
 constexpr int MOUT = 2 * TIN;                  // outputs per tile = UMMA M
@@ -59,7 +62,8 @@ constexpr int EPI_WARPS = 4;
 constexpr int THREADS = (LOADER_WARPS + EPI_WARPS + 1) * 32;   // loader warps, epilogue warps, 1 MMA warp (416: 128 registers each)
 constexpr int PREFETCH = 4;                    // chunks of global loads in flight per loader thread (64 KB per CTA)
 constexpr int TMEM_COLS = 512;
-constexpr int COL_THI = 0, COL_TLO = KWIN, COL_D = 2 * KWIN;   // two accumulator buffers of NR columns at COL_D: 320 + 2 * 96 = 512
+constexpr int COL_THI = 0, COL_TLO = KWIN, COL_D = 2 * KWIN;   // accumulator buffer(s) of NR columns at COL_D
+constexpr int NBUF = (2 * KWIN + 2 * NR <= TMEM_COLS) ? 2 : 1;  // 48-row strips: 320 + 2 x 96 = 512 columns; 64-row strips: 320 + 128
 
 struct UpTcArgs {
     const float2* in;        // [rows][n_in]
@@ -123,6 +127,11 @@ __device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t (&v)[16])
                  : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
                    "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
                  : "r"(taddr));
+}
+__device__ __forceinline__ void tmem_ld8(uint32_t taddr, uint32_t (&v)[8])
+{
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
+                 : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]) : "r"(taddr));
 }
 __device__ __forceinline__ void tmem_st32(uint32_t taddr, const uint32_t (&v)[32])
 {
@@ -309,7 +318,7 @@ __global__ void __launch_bounds__(THREADS, 1) spiir_up2_tc_kernel(const UpTcArgs
                 for (int j = 0; j < J; ++j) {
                     const int cn = cbase + 2 * j + WIN_CH - 1;          // newest chunk of this tile's window
                     bar_wait(full(cn % RING_CH), (uint32_t)((cn / RING_CH) & 1));
-                    const int t = tbase + j, buf = t & 1, use = t >> 1;
+                    const int t = tbase + j, buf = t % NBUF, use = t / NBUF;
                     if (use > 0) bar_wait(tempty(buf), (uint32_t)((use - 1) & 1));   // this buffer's previous tile has been drained
                     const uint32_t d = tmem + COL_D + (uint32_t)(buf * NR);
                     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
@@ -340,40 +349,44 @@ __global__ void __launch_bounds__(THREADS, 1) spiir_up2_tc_kernel(const UpTcArgs
             const int ew = warp & 3;
             const int tl = ew * 32 + lane;                              // output index within the tile
             for (int j = 0; j < J; ++j) {
-                const int t = tbase + j, buf = t & 1, use = t >> 1;
+                const int t = tbase + j, buf = t % NBUF, use = t / NBUF;
                 const int m0 = ms + j * TIN;
                 const bool tok = tl < 2 * min(TIN, a.n_in - m0);
                 float2* obase = a.out + (size_t)row0 * 2 * a.n_in + 2 * m0 + tl;
                 const uint32_t taddr = tmem + ((uint32_t)(ew * 32) << 16) + COL_D + (uint32_t)(buf * NR);
                 bar_wait(tfull(buf), (uint32_t)(use & 1));
                 asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-                uint32_t vre[ROWS / 16][16], vim[ROWS / 16][16];
+                // drain in two halves (ROWS registers each); the buffer is released right after the second drain
 #pragma unroll
-                for (int hh = 0; hh < ROWS / 16; ++hh) {
-                    tmem_ld16(taddr + 16 * hh, vre[hh]);
-                    tmem_ld16(taddr + ROWS + 16 * hh, vim[hh]);
-                }
-                asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-                asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
-                __syncwarp();
-                if (lane == 0) bar_arrive(tempty(buf));
-                // accumulate = a vector reduction performed by the L2 (one addend per element and call: deterministic);
-                // no read-modify-write round trip through this thread's registers
+                for (int h2 = 0; h2 < 2; ++h2) {
+                    constexpr int RH = ROWS / 2;                        // rows per half (multiple of 8)
+                    uint32_t vre[RH], vim[RH];
 #pragma unroll
-                for (int hh = 0; hh < ROWS / 16; ++hh) {
-                    float2* ob = obase + (size_t)(16 * hh) * 2 * a.n_in;
-                    const int rbase = row0 + 16 * hh;
+                    for (int q8 = 0; q8 < RH / 8; ++q8) {
+                        tmem_ld8(taddr + RH * h2 + 8 * q8, *reinterpret_cast<uint32_t (*)[8]>(&vre[8 * q8]));
+                        tmem_ld8(taddr + ROWS + RH * h2 + 8 * q8, *reinterpret_cast<uint32_t (*)[8]>(&vim[8 * q8]));
+                    }
+                    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+                    if (h2 == 1) {
+                        asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+                        __syncwarp();
+                        if (lane == 0) bar_arrive(tempty(buf));
+                    }
+                    // accumulate = a vector reduction performed by the L2 (one addend per element and call: deterministic);
+                    // no read-modify-write round trip through this thread's registers
+                    float2* ob = obase + (size_t)(RH * h2) * 2 * a.n_in;
+                    const int rbase = row0 + RH * h2;
                     if (a.accumulate) {
 #pragma unroll
-                        for (int i = 0; i < 16; ++i)
+                        for (int i = 0; i < RH; ++i)
                             if (tok && rbase + i < a.rows)
                                 asm volatile("red.global.add.v2.f32 [%0], {%1, %2};" ::"l"(ob + (size_t)i * 2 * a.n_in),
-                                             "f"(__uint_as_float(vre[hh][i])), "f"(__uint_as_float(vim[hh][i])) : "memory");
+                                             "f"(__uint_as_float(vre[i])), "f"(__uint_as_float(vim[i])) : "memory");
                     } else {
 #pragma unroll
-                        for (int i = 0; i < 16; ++i)
+                        for (int i = 0; i < RH; ++i)
                             if (tok && rbase + i < a.rows)
-                                ob[(size_t)i * 2 * a.n_in] = make_float2(__uint_as_float(vre[hh][i]), __uint_as_float(vim[hh][i]));
+                                ob[(size_t)i * 2 * a.n_in] = make_float2(__uint_as_float(vre[i]), __uint_as_float(vim[i]));
                     }
                 }
             }
