@@ -1,8 +1,8 @@
 // spiir_resample_tc.cuh -- up-by-2 (+ accumulate) with the 192-tap FIR on the 5th-generation tensor cores
 // (row a10 of SURVEY.md section 8; Eq. 9).
 //
-// The polyphase FIR  w[2m+p] = 2 sum_{q<96} h[2q+p] v[m-q]  of a strip of 64 complex rows is a dense contraction
-// with a banded Toeplitz matrix; a strip is 48 complex rows, one tile = 64 input positions -> 128 outputs:
+// The polyphase FIR  w[2m+p] = 2 sum_{q<96} h[2q+p] v[m-q]  of a strip of rows is a dense contraction with a banded
+// Toeplitz matrix; a strip is 48 complex rows, one tile = 64 input positions -> 128 outputs:
 //     D[t, row'] = sum_k T[t, k] * X[row', k]
 //   T: 128 outputs of the tile x a window of K = 160 input samples (96 before the tile + its 64 inputs),
 //      T[2m'+p, k] = 2 h[2 (96 + m' - k) + p] for 1 <= k - m' <= 96, zero elsewhere (60 % dense).  It is the same for
@@ -59,8 +59,8 @@ constexpr int OFF_TPTR = OFF_BAR + NBAR * 8;
 constexpr int SMEM_BYTES = OFF_TPTR + 16;
 constexpr int LOADER_WARPS = ROWS / 8;         // a loader warp owns 8 rows
 constexpr int EPI_WARPS = 4;
-constexpr int THREADS = (LOADER_WARPS + EPI_WARPS + 1) * 32;   // loader warps, epilogue warps, 1 MMA warp (416: 128 registers each)
-constexpr int PREFETCH = 4;                    // chunks of global loads in flight per loader thread (64 KB per CTA)
+constexpr int THREADS = (LOADER_WARPS + EPI_WARPS + 1) * 32;   // loader warps, epilogue warps, 1 MMA warp (352 threads at 48 rows)
+constexpr int PREFETCH = 4;                    // chunks of global loads in flight per loader thread (48 KB per CTA; 6 measured no faster)
 constexpr int TMEM_COLS = 512;
 constexpr int COL_THI = 0, COL_TLO = KWIN, COL_D = 2 * KWIN;   // accumulator buffer(s) of NR columns at COL_D
 constexpr int NBUF = (2 * KWIN + 2 * NR <= TMEM_COLS) ? 2 : 1;  // 48-row strips: 320 + 2 x 96 = 512 columns; 64-row strips: 320 + 128
