@@ -31,27 +31,35 @@ spiir_status device_info(DeviceInfo* out)
 }
 
 // cudaFuncSetAttribute costs several microseconds of host time: raise a kernel's dynamic shared memory
-// limit only when a launch needs more than any earlier one did (per device the limit only grows).
+// limit only when a launch needs more than any earlier one did (per device the limit only grows); the first call for a
+// kernel also fixes its shared-memory carveout.
 cudaError_t ensure_smem(const void* func, int bytes)
 {
     static std::mutex mu;
     static const void* funcs[512];
     static int devs[512], limits[512];
     static int nfuncs = 0;
-    if (bytes <= 48 * 1024) return cudaSuccess;          // the default limit
     int dev = 0;
-    cudaError_t e = cudaGetDevice(&dev);                 // the attribute is per device
+    cudaError_t e = cudaGetDevice(&dev);                 // the attributes are per device
     if (e != cudaSuccess) return e;
     std::lock_guard<std::mutex> lock(mu);
+    int slot = -1;
     for (int i = 0; i < nfuncs; ++i)
-        if (funcs[i] == func && devs[i] == dev) {
-            if (limits[i] >= bytes) return cudaSuccess;
-            e = cudaFuncSetAttribute(func, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
-            if (e == cudaSuccess) limits[i] = bytes;
-            return e;
-        }
+        if (funcs[i] == func && devs[i] == dev) { slot = i; break; }
+    if (slot < 0) {
+        // First launch of this kernel on this device: every kernel of the library asks for the SAME shared-memory carveout
+        // (the maximum).  Kernels whose preferred L1 / shared split differs do not share an SM, and the multirate plan runs
+        // its per-rate banks side by side on forked streams: with the default (per-kernel) carveouts they ran one after the
+        // other (109 us for the six lower banks of configs[3] = the sum of their times).
+        e = cudaFuncSetAttribute(func, cudaFuncAttributePreferredSharedMemoryCarveout, (int)cudaSharedmemCarveoutMaxShared);
+        if (e != cudaSuccess) return e;
+        if (nfuncs >= 512) return bytes <= 48 * 1024 ? cudaSuccess : cudaFuncSetAttribute(func, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+        slot = nfuncs++;
+        funcs[slot] = func; devs[slot] = dev; limits[slot] = 48 * 1024;
+    }
+    if (bytes <= limits[slot]) return cudaSuccess;
     e = cudaFuncSetAttribute(func, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
-    if (e == cudaSuccess && nfuncs < 512) { funcs[nfuncs] = func; devs[nfuncs] = dev; limits[nfuncs] = bytes; ++nfuncs; }
+    if (e == cudaSuccess) limits[slot] = bytes;
     return e;
 }
 
