@@ -103,6 +103,33 @@ static spiir_status launch_down_fir(spiir_resamp* r, const DownArgs& d, size_t s
     return SPIIR_OK;
 }
 
+// Tensor map of one call's input [rows][n_in] complex64, seen as rows of 2 n_in floats; box = 32 floats (16 samples) x
+// ROWS rows with the 128-byte swizzle, zero fill outside the tensor.  cuTensorMapEncodeTiled is a host-side encoder (no
+// driver call on the stream); it is resolved through the runtime so that the library does not link against libcuda.
+static spiir_status up_tc_tensor_map(CUtensorMap* map, const void* in, int rows, int n_in)
+{
+    typedef CUresult (*encode_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+    static encode_fn encode = nullptr;
+    if (!encode) {
+        void* fn = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        SPIIR_CUDA(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &q));
+        if (!fn || q != cudaDriverEntryPointSuccess) { set_error("cuTensorMapEncodeTiled is not available"); return SPIIR_ECUDA; }
+        encode = reinterpret_cast<encode_fn>(fn);
+    }
+    const cuuint64_t dims[2] = {(cuuint64_t)2 * n_in, (cuuint64_t)rows};
+    const cuuint64_t strides[1] = {(cuuint64_t)n_in * 8};
+    const cuuint32_t box[2] = {32, (cuuint32_t)tc::ROWS};
+    const cuuint32_t estr[2] = {1, 1};
+    const CUresult rc = encode(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, const_cast<void*>(in), dims, strides, box, estr,
+                               CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (rc != CUDA_SUCCESS) { set_error("cuTensorMapEncodeTiled failed (%d)", (int)rc); return SPIIR_ECUDA; }
+    return SPIIR_OK;
+}
+
 template <int HALF>
 static void fill_up_taps(const spiir_resamp* r, UpTaps<HALF>* t)
 {
@@ -255,9 +282,15 @@ spiir_status spiir_resample_up(spiir_resamp_t* r, const spiir_c64* in, int n_in,
         t.seg_tiles = (t.tiles_per_row + nsegs - 1) / nsegs;
         t.nsegs = (t.tiles_per_row + t.seg_tiles - 1) / t.seg_tiles;
         t.in16 = ((reinterpret_cast<uintptr_t>(in) & 15u) == 0 && (n_in & 1) == 0) ? 1 : 0;
+        CUtensorMap in_map;
+        memset(&in_map, 0, sizeof in_map);
+        if (t.in16) {
+            spiir_status mrc = up_tc_tensor_map(&in_map, in, r->rows, n_in);
+            if (mrc != SPIIR_OK) return mrc;
+        }
         const int grid = std::min(t.nstrips * t.nsegs, r->dev.n_sm);
         SPIIR_CUDA(ensure_smem((const void*)tc::spiir_up2_tc_kernel, tc::SMEM_BYTES));
-        tc::spiir_up2_tc_kernel<<<grid, tc::THREADS, tc::SMEM_BYTES, st>>>(t);
+        tc::spiir_up2_tc_kernel<<<grid, tc::THREADS, tc::SMEM_BYTES, st>>>(t, in_map);
         SPIIR_CUDA(cudaGetLastError());
         return SPIIR_OK;
     }

@@ -20,12 +20,15 @@
 // is 5 consecutive chunks, every tile advances it by two and two chunks are free for the loader to run a whole tile
 // ahead; each input sample is written to shared memory once and read by 2.5 tiles; a K = 8 instruction takes two adjacent units and never straddles the ring's end.
 //
-// Roles (352 threads): warps 0-5 load + split + store the data chunks (8 rows per warp, global loads prefetched four
-// chunks deep in registers), warp 10 issues the MMAs (one thread) and owns TMEM, warps 6-9 drain the accumulator (tcgen05.ld):
-// a lane is an output sample, so a warp writes 256 contiguous bytes of one row per store -- no transposition; with
-// accumulate the store is a vector reduction (red.global.add.v2.f32) done by the L2.  mbarriers: full[7] /
-// empty[7] per ring chunk, tfull[2] / tempty[2] for the accumulator buffers.  CTAs are persistent over (strip, time segment) units.
+// Roles (384 threads): one thread of warp 11 fetches the raw chunks (ROWS rows x 32 samples) with TMA tile copies through
+// a tensor map of the input into a 4-slot staging ring (48 KB of loads in flight per SM); warps 0-5 read a staged chunk,
+// split it into TF32 high / low parts and store it as the data operand; warp 10 issues the MMAs (one thread) and owns
+// TMEM; warps 6-9 drain the accumulator (tcgen05.ld): a lane is an output sample, so a warp writes 256 contiguous bytes of
+// one row per store -- no transposition; with accumulate the store is a vector reduction (red.global.add.v2.f32) done
+// by the L2.  mbarriers: sfull[4] / sempty[4] per staging slot, full[7] / empty[7] per ring chunk, tfull[2] / tempty[2]
+// for the accumulator buffers.  CTAs are persistent over (strip, time segment) units.
 #pragma once
+#include <cuda.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
 
@@ -37,7 +40,7 @@ namespace tc {
 #ifndef SPIIR_TC_ROWS
 #define SPIIR_TC_ROWS 48
 #endif
-constexpr int ROWS = SPIIR_TC_ROWS;            // complex rows per strip: 48 (double-buffered accumulator; 327 us) or 64 (N = 128, single buffer; 375 us)
+constexpr int ROWS = SPIIR_TC_ROWS;            // complex rows per strip: 48 (double-buffered accumulator); 64 (N = 128) leaves one buffer and measured slower
 constexpr int NR = 2 * ROWS;                   // real rows = UMMA N
 constexpr int TIN = 64;                        // input samples per tile
 constexpr int MOUT = 2 * TIN;                  // outputs per tile = UMMA M
@@ -53,14 +56,22 @@ constexpr int RING_UNITS = RING_CH * CHU;      // 56 (even)
 constexpr int UNIT_BYTES = NR * 16;
 constexpr int PART_BYTES = RING_UNITS * UNIT_BYTES;
 constexpr int OFF_LO = PART_BYTES;
-constexpr int OFF_BAR = 2 * PART_BYTES;
-constexpr int NBAR = 2 * RING_CH + 4;
+constexpr int STG_SLOTS = 4;                   // raw chunks in flight per CTA (TMA tensor copies, 48 KB)
+constexpr int STG_HALF = ROWS * 128;           // half a chunk: ROWS x 16 samples = ROWS x 128 bytes, 128-byte swizzle
+constexpr int STG_BYTES = 2 * STG_HALF;
+static_assert(STG_HALF % 1024 == 0 && (2 * PART_BYTES) % 1024 == 0, "the 128-byte swizzle pattern repeats every 1024 bytes");
+constexpr int OFF_STG = 2 * PART_BYTES;
+constexpr int OFF_BAR = OFF_STG + STG_SLOTS * STG_BYTES;
+constexpr int NBAR = 2 * RING_CH + 4 + 2 * STG_SLOTS;
 constexpr int OFF_TPTR = OFF_BAR + NBAR * 8;
 constexpr int SMEM_BYTES = OFF_TPTR + 16;
-constexpr int LOADER_WARPS = ROWS / 8;         // a loader warp owns 8 rows
+constexpr int LOADER_WARPS = ROWS / 8;         // warps that split and store the data operand
+constexpr int LOADERS = LOADER_WARPS * 32;
 constexpr int EPI_WARPS = 4;
-constexpr int THREADS = (LOADER_WARPS + EPI_WARPS + 1) * 32;   // loader warps, epilogue warps, 1 MMA warp (352 threads at 48 rows)
-constexpr int PREFETCH = 4;                    // chunks of global loads in flight per loader thread (48 KB per CTA; 6 measured no faster)
+constexpr int THREADS = (LOADER_WARPS + EPI_WARPS + 2) * 32;   // loader warps, epilogue warps, 1 MMA warp, 1 TMA warp (384 threads at 48 rows)
+constexpr int ITEMS = ROWS * CHU / LOADERS;    // (row, unit) items of a chunk per loader thread
+static_assert(ROWS * CHU % LOADERS == 0, "a chunk must split evenly over the loader threads");
+static_assert(SMEM_BYTES <= 227 * 1024, "shared memory");
 constexpr int TMEM_COLS = 512;
 constexpr int COL_THI = 0, COL_TLO = KWIN, COL_D = 2 * KWIN;   // accumulator buffer(s) of NR columns at COL_D
 constexpr int NBUF = (2 * KWIN + 2 * NR <= TMEM_COLS) ? 2 : 1;  // 48-row strips: 320 + 2 x 96 = 512 columns; 64-row strips: 320 + 128
@@ -146,6 +157,22 @@ __device__ __forceinline__ void sts128(uint32_t addr, float4 v)
 {
     asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w) : "memory");
 }
+__device__ __forceinline__ float4 lds128(uint32_t addr)
+{
+    float4 v;
+    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr) : "memory");
+    return v;
+}
+__device__ __forceinline__ void bar_expect_tx(uint32_t bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+// TMA tile copy global -> shared through a 2-D tensor map (box = 32 floats x ROWS rows); completion is counted on the mbarrier
+__device__ __forceinline__ void tma_g2s_2d(uint32_t dst, const CUtensorMap* map, int c0, int c1, uint32_t bar)
+{
+    asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
+                 ::"r"(dst), "l"(map), "r"(c0), "r"(c1), "r"(bar) : "memory");
+}
 __device__ __forceinline__ void umma_commit(uint32_t bar)
 {
     asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
@@ -165,7 +192,7 @@ __device__ __forceinline__ float2 sample_at(const float2* in_row, const float2* 
 }
 
 
-__global__ void __launch_bounds__(THREADS, 1) spiir_up2_tc_kernel(const UpTcArgs a)
+__global__ void __launch_bounds__(THREADS, 1) spiir_up2_tc_kernel(const UpTcArgs a, const __grid_constant__ CUtensorMap in_map)
 {
     extern __shared__ __align__(1024) unsigned char sm[];
     const uint32_t sbase = s32(sm);
@@ -174,6 +201,8 @@ __global__ void __launch_bounds__(THREADS, 1) spiir_up2_tc_kernel(const UpTcArgs
     auto empty = [&](int i) { return bar0 + 8u * (uint32_t)(RING_CH + i); };
     auto tfull = [&](int i) { return bar0 + 8u * (uint32_t)(2 * RING_CH + i); };
     auto tempty = [&](int i) { return bar0 + 8u * (uint32_t)(2 * RING_CH + 2 + i); };
+    auto sfull = [&](int i) { return bar0 + 8u * (uint32_t)(2 * RING_CH + 4 + i); };
+    auto sempty = [&](int i) { return bar0 + 8u * (uint32_t)(2 * RING_CH + 4 + STG_SLOTS + i); };
     uint32_t* tptr = reinterpret_cast<uint32_t*>(sm + OFF_TPTR);
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int ph = phase_read(a.phase);
@@ -184,6 +213,7 @@ __global__ void __launch_bounds__(THREADS, 1) spiir_up2_tc_kernel(const UpTcArgs
     if (tid == 0) {
         for (int i = 0; i < RING_CH; ++i) { bar_init(full(i), LOADER_WARPS); bar_init(empty(i), 1); }
         for (int i = 0; i < 2; ++i) { bar_init(tfull(i), 1); bar_init(tempty(i), EPI_WARPS); }
+        for (int i = 0; i < STG_SLOTS; ++i) { bar_init(sfull(i), 1); bar_init(sempty(i), LOADER_WARPS); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     if (warp == LOADER_WARPS + EPI_WARPS) {
@@ -220,7 +250,7 @@ __global__ void __launch_bounds__(THREADS, 1) spiir_up2_tc_kernel(const UpTcArgs
     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
 
     const int nunits = a.nstrips * a.nsegs;
-    int cbase = 0, tbase = 0;                                          // chunks / tiles of this CTA's earlier units
+    int cbase = 0, tbase = 0, sbase_ch = 0;                            // chunks / tiles / staged chunks of this CTA's earlier units
     for (int u = blockIdx.x; u < nunits; u += gridDim.x) {
         const int strip = u / a.nsegs, seg = u % a.nsegs;
         const int tile0 = seg * a.seg_tiles;
@@ -229,25 +259,28 @@ __global__ void __launch_bounds__(THREADS, 1) spiir_up2_tc_kernel(const UpTcArgs
         const int row0 = strip * ROWS;
         const int nch = WIN_CH - 2 + 2 * J;                            // chunks of this unit: 3 of halo + 2 per tile
 
+        // A chunk that lies inside the block with 16-byte aligned rows is STAGED: one thread fetches its raw samples with
+        // two TMA tile copies (ROWS rows x 16 samples each, through the tensor map of `in`) into a ring of STG_SLOTS slots,
+        // so STG_SLOTS chunks of DRAM latency are in flight whatever the loader warps are doing.  (Loads prefetched in
+        // registers were not: ptxas gave every prefetch batch the same scoreboard, so waiting for the oldest batch waited
+        // for the newest; one bulk copy per row was no better: the TMA unit took ~70 cycles per 256-byte request.)
+        // Other chunks (history in front of the block, ragged end, unaligned rows) are read element by element.
+        auto staged = [&](int ci) {
+            const int mc = ms - HALF + ci * CHS;
+            return a.in16 && mc >= 0 && mc + CHS <= a.n_in;
+        };
         if (warp < LOADER_WARPS) {
-            // ===== loaders: 64 rows x 32 samples per chunk.  A warp owns 8 rows; lane = (row, piece): every load instruction
-            // reads 4 consecutive 16-byte pieces (64 contiguous bytes) of each of its 8 rows, so the L1 sees 8 line requests
-            // per instruction instead of 32.  A piece is two samples = half a unit: lane pairs (piece, piece ^ 1) swap halves
-            // so that the even lane ends up with re[4] and the odd lane with im[4] of one unit; a quarter warp then stores
-            // 8 different rows of one unit: conflict-free 16-byte stores. =====
-            const int rowlow = lane & 7, piece = lane >> 3;
-            const int r = warp * 8 + rowlow;
-            const bool odd = (piece & 1) != 0;
-            const int row = row0 + r;
-            const bool rowok = row < a.rows;
-            const float2* in_row = a.in + (size_t)(rowok ? row : 0) * a.n_in;
-            const float2* hist_row = hcur + (size_t)(rowok ? row : 0) * (HALF - 1);
-            // Carried history of this strip's rows = the last 95 samples of (history ++ block).  A block of at least 95 samples
-            // supplies all of them, and they pass through this thread's registers anyway (written below); shorter blocks
-            // take this explicit copy.
+            // ===== loaders: split a chunk (ROWS x 32 samples) into TF32 high / low parts and store it as the MMA's data operand.
+            // Thread item = (row r, unit u): 4 consecutive samples of one row = two 16-byte reads from the staging slot
+            // (consecutive lanes = consecutive rows; the 128-byte swizzle puts piece j of row r at j ^ (r mod 8):
+            // conflict-free) and, after the split, four 16-byte stores (re / im, high / low; consecutive lanes =
+            // consecutive 16-byte slots of one unit: conflict-free). =====
             const int hfirst = a.n_in - (HALF - 1);                     // first block sample that is part of the next history
+            // Carried history of this strip's rows = the last 95 samples of (history ++ block).  A block of at least 95 samples
+            // supplies all of them, and they pass through the loaders' registers anyway (written below); shorter blocks
+            // take this explicit copy.
             if (seg == 0 && hfirst < 0) {
-                for (int i = tid; i < ROWS * (HALF - 1); i += LOADER_WARPS * 32) {
+                for (int i = tid; i < ROWS * (HALF - 1); i += LOADERS) {
                     const int rr = i / (HALF - 1), k = i % (HALF - 1), rw = row0 + rr;
                     if (rw < a.rows) {
                         const int g = a.n_in - (HALF - 1) + k;
@@ -256,60 +289,97 @@ __global__ void __launch_bounds__(THREADS, 1) spiir_up2_tc_kernel(const UpTcArgs
                     }
                 }
             }
-            // rolling software prefetch: the loads of chunk ci + PREFETCH are issued as soon as chunk ci's registers
-            // have been consumed, so PREFETCH chunks stay in flight while this thread waits for ring space
-            float4 q[PREFETCH][4];                                      // pieces piece, piece + 4, piece + 8, piece + 12 of the chunk
-            auto issue = [&](int ci, float4 (&dst)[4]) {
+            int sc = sbase_ch;
+            for (int ci = 0; ci < nch; ++ci) {
+                const int c = cbase + ci, slot = c % RING_CH, fill = c / RING_CH;
                 const int mc = ms - HALF + ci * CHS;                    // first sample of the chunk
-                if (ci < nch && rowok && mc >= 0 && mc + CHS <= a.n_in && a.in16) {
-                    const float4* p = reinterpret_cast<const float4*>(in_row + mc) + piece;
+                const bool stg = staged(ci);
+                const int ss = sc % STG_SLOTS;
+                float4 v[ITEMS][2];                                     // (re, im) of samples 4u .. 4u + 3 of row r
+                if (stg) {
+                    bar_wait(sfull(ss), (uint32_t)((sc / STG_SLOTS) & 1));
 #pragma unroll
-                    for (int i = 0; i < 4; ++i) dst[i] = p[4 * i];
+                    for (int k = 0; k < ITEMS; ++k) {
+                        const int idx = tid + k * LOADERS, r = idx % ROWS, u = idx / ROWS;
+                        const uint32_t src = sbase + OFF_STG + (uint32_t)(ss * STG_BYTES + (u >> 2) * STG_HALF + r * 128);
+                        const int j = 2 * (u & 3), x = r & 7;
+                        v[k][0] = lds128(src + (uint32_t)((j ^ x) << 4));
+                        v[k][1] = lds128(src + (uint32_t)(((j + 1) ^ x) << 4));
+                    }
+                    __syncwarp();
+                    if (lane == 0) bar_arrive(sempty(ss));              // the slot may be refilled
+                    ++sc;
                 } else {
 #pragma unroll
-                    for (int i = 0; i < 4; ++i) {
-                        float2 s0 = make_float2(0.f, 0.f), s1 = s0;
-                        const int m = mc + 2 * (4 * i + piece);
-                        if (ci < nch && rowok) { s0 = sample_at(in_row, hist_row, m, a.n_in); s1 = sample_at(in_row, hist_row, m + 1, a.n_in); }
-                        dst[i] = make_float4(s0.x, s0.y, s1.x, s1.y);
+                    for (int k = 0; k < ITEMS; ++k) {
+                        const int idx = tid + k * LOADERS, r = idx % ROWS, u = idx / ROWS;
+                        const int row = row0 + r, m = mc + 4 * u;
+                        float2 q[4];
+#pragma unroll
+                        for (int e = 0; e < 4; ++e) q[e] = make_float2(0.f, 0.f);
+                        if (row < a.rows) {
+                            const float2* in_row = a.in + (size_t)row * a.n_in;
+                            const float2* hist_row = hcur + (size_t)row * (HALF - 1);
+#pragma unroll
+                            for (int e = 0; e < 4; ++e) q[e] = sample_at(in_row, hist_row, m + e, a.n_in);
+                        }
+                        v[k][0] = make_float4(q[0].x, q[0].y, q[1].x, q[1].y);
+                        v[k][1] = make_float4(q[2].x, q[2].y, q[3].x, q[3].y);
                     }
                 }
-            };
+                // the next history = the block's last 95 samples: written by the unit that owns them (not from a halo)
+                if (ci >= HALO_CH && hfirst >= 0 && mc + CHS > hfirst) {
 #pragma unroll
-            for (int pi = 0; pi < PREFETCH; ++pi) issue(pi, q[pi]);
-            for (int c0 = 0; c0 < nch; c0 += PREFETCH) {
+                    for (int k = 0; k < ITEMS; ++k) {
+                        const int idx = tid + k * LOADERS, r = idx % ROWS, u = idx / ROWS;
+                        const int row = row0 + r, g = mc + 4 * u - hfirst;
+                        if (row < a.rows) {
+                            float2* hrow = hnext + (size_t)row * (HALF - 1);
+                            const float2 q[4] = {make_float2(v[k][0].x, v[k][0].y), make_float2(v[k][0].z, v[k][0].w),
+                                                 make_float2(v[k][1].x, v[k][1].y), make_float2(v[k][1].z, v[k][1].w)};
 #pragma unroll
-                for (int pi = 0; pi < PREFETCH; ++pi) {
-                    const int ci = c0 + pi;
-                    if (ci < nch) {                                      // uniform over the CTA's loader threads
-                        const int c = cbase + ci, slot = c % RING_CH, fill = c / RING_CH;
-                        if (fill > 0) bar_wait(empty(slot), (uint32_t)((fill - 1) & 1));
-#pragma unroll
-                        for (int i = 0; i < 4; ++i) {
-                            const float4 v = q[pi][i];                  // (re, im) of samples 2 (4i + piece), +1
-                            if (ci >= HALO_CH && hfirst >= 0 && rowok) {
-                                const int g = ms - HALF + ci * CHS + 2 * (4 * i + piece) - hfirst;
-                                float2* hrow = hnext + (size_t)row * (HALF - 1);
-                                if (g >= 0 && g < HALF - 1) hrow[g] = make_float2(v.x, v.y);
-                                if (g + 1 >= 0 && g + 1 < HALF - 1) hrow[g + 1] = make_float2(v.z, v.w);
-                            }
-                            const float rx = __shfl_xor_sync(0xffffffffu, odd ? v.x : v.y, 8);
-                            const float ry = __shfl_xor_sync(0xffffffffu, odd ? v.z : v.w, 8);
-                            const float4 w = odd ? make_float4(rx, ry, v.y, v.w) : make_float4(v.x, v.z, rx, ry);   // im[4] : re[4]
-                            const float4 wh = make_float4(tf32_hi(w.x), tf32_hi(w.y), tf32_hi(w.z), tf32_hi(w.w));
-                            const float4 wl = make_float4(w.x - wh.x, w.y - wh.y, w.z - wh.z, w.w - wh.w);
-                            const uint32_t addr = sbase + (uint32_t)(slot * CHU + 2 * i + (piece >> 1)) * UNIT_BYTES +
-                                                  (uint32_t)((odd ? ROWS : 0) + r) * 16;
-                            sts128(addr, wh);
-                            sts128(addr + OFF_LO, wl);
+                            for (int e = 0; e < 4; ++e)
+                                if (g + e >= 0 && g + e < HALF - 1 && mc + 4 * u + e < a.n_in) hrow[g + e] = q[e];
                         }
-                        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-                        __syncwarp();
-                        if (lane == 0) bar_arrive(full(slot));          // one arrival per warp
-                        issue(ci + PREFETCH, q[pi]);
                     }
+                }
+                if (fill > 0) bar_wait(empty(slot), (uint32_t)((fill - 1) & 1));
+#pragma unroll
+                for (int k = 0; k < ITEMS; ++k) {
+                    const int idx = tid + k * LOADERS, r = idx % ROWS, u = idx / ROWS;
+                    const float4 wre = make_float4(v[k][0].x, v[k][0].z, v[k][1].x, v[k][1].z);
+                    const float4 wim = make_float4(v[k][0].y, v[k][0].w, v[k][1].y, v[k][1].w);
+                    const float4 hre = make_float4(tf32_hi(wre.x), tf32_hi(wre.y), tf32_hi(wre.z), tf32_hi(wre.w));
+                    const float4 him = make_float4(tf32_hi(wim.x), tf32_hi(wim.y), tf32_hi(wim.z), tf32_hi(wim.w));
+                    const uint32_t addr = sbase + (uint32_t)(slot * CHU + u) * UNIT_BYTES + (uint32_t)r * 16;
+                    sts128(addr, hre);
+                    sts128(addr + ROWS * 16, him);
+                    sts128(addr + OFF_LO, make_float4(wre.x - hre.x, wre.y - hre.y, wre.z - hre.z, wre.w - hre.w));
+                    sts128(addr + OFF_LO + ROWS * 16, make_float4(wim.x - him.x, wim.y - him.y, wim.z - him.z, wim.w - him.w));
+                }
+                asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+                __syncwarp();
+                if (lane == 0) bar_arrive(full(slot));                  // one arrival per warp
+            }
+        } else
+        if (warp == LOADER_WARPS + EPI_WARPS + 1) {
+            // ===== copy thread: two tile copies per staged chunk, up to STG_SLOTS chunks ahead of the loaders.  Rows past the
+            // end of the batch are zero-filled by the TMA unit (and count in the transaction bytes). =====
+            if (lane == 0) {
+                int sc = sbase_ch;
+                for (int ci = 0; ci < nch; ++ci) {
+                    if (!staged(ci)) continue;
+                    const int ss = sc % STG_SLOTS, f = sc / STG_SLOTS;
+                    if (f > 0) bar_wait(sempty(ss), (uint32_t)((f - 1) & 1));
+                    bar_expect_tx(sfull(ss), (uint32_t)STG_BYTES);
+                    const int c0 = 2 * (ms - HALF + ci * CHS);          // float index of the chunk's first sample
+                    const uint32_t dst = sbase + OFF_STG + (uint32_t)(ss * STG_BYTES);
+                    tma_g2s_2d(dst, &in_map, c0, row0, sfull(ss));
+                    tma_g2s_2d(dst + STG_HALF, &in_map, c0 + 32, row0, sfull(ss));
+                    ++sc;
                 }
             }
+            __syncwarp();
         } else
         if (warp == LOADER_WARPS + EPI_WARPS) {
             // ===== MMA issuer (one thread) =====
@@ -391,6 +461,7 @@ __global__ void __launch_bounds__(THREADS, 1) spiir_up2_tc_kernel(const UpTcArgs
                 }
             }
         }
+        for (int ci = 0; ci < nch; ++ci) sbase_ch += staged(ci) ? 1 : 0;
         cbase += nch;
         tbase += J;
     }
