@@ -194,7 +194,8 @@ spiir_status plan_geometry(const spiir_plan* p, const spiir_bank_class& c, int n
 static void fill_filter_args(const spiir_plan* p, const spiir_bank_class& c, const float* x, int n, spiir_c64* z, int accumulate,
                              const FilterGeometry& g, FilterArgs* a)
 {
-    a->coef = c.d_coef; a->dly = c.d_dly; a->state = p->d_state + c.state_off; a->sstride = p->nfilt_total;
+    a->coef = c.d_coef; a->dly = c.d_dly; a->apow = (g.scan && c.d_apow && g.C == c.apow_C) ? c.d_apow : nullptr;
+    a->state = p->d_state + c.state_off; a->sstride = p->nfilt_total;
     a->chunk_st = c.d_chunk;
     a->hbuf[0] = p->d_hist[0]; a->hbuf[1] = p->d_hist[1]; a->phase = p->d_phase;
     a->x = x; a->z = reinterpret_cast<float2*>(z);
@@ -320,6 +321,7 @@ size_t plan_layout(spiir_plan* p, Arena* a)
     for (spiir_bank_class& c : p->cls) {
         c.d_coef = a->take_n<float4>(c.nfilt);
         c.d_dly = a->take_n<int32_t>(c.nfilt);
+        c.d_apow = scan_mapping_supported(c.F, c.LPT, c.NP) ? a->take_n<float2>(c.nfilt) : nullptr;
         c.d_tmap = p->L_uniform ? nullptr : a->take_n<int32_t>((size_t)c.T);
         c.d_chunk = c.NC_cap > 1 ? a->take_n<float2>((size_t)c.NC_cap * p->S * c.nfilt) : nullptr;
     }
@@ -458,6 +460,22 @@ spiir_status plan_create_in(spiir_plan_t** out, const spiir_c64* a1, const spiir
             if (cpos[i] >= 0) pos[i] = (int32_t)(c.state_off + (size_t)cpos[i]);
         SPIIR_TRY(cudaMemcpy(c.d_coef, coef.data(), c.nfilt * sizeof(float4), cudaMemcpyHostToDevice));
         SPIIR_TRY(cudaMemcpy(c.d_dly, dly.data(), c.nfilt * sizeof(int32_t), cudaMemcpyHostToDevice));
+        if (c.d_apow) {
+            // chunk carry factor of the in-CTA scan at the plan's block length: a1^C in double, rounded once
+            FilterGeometry g;
+            c.apow_C = 0;
+            if (plan_geometry(p, c, p->max_block, &g) == SPIIR_OK && g.scan) c.apow_C = g.C;
+            std::vector<float> apow(c.nfilt * 2, 0.f);
+            for (size_t i = 0; i < c.nfilt && c.apow_C > 0; ++i) {
+                double pr = 1.0, pi = 0.0, br = (double)coef[4 * i], bi = (double)coef[4 * i + 1];
+                for (int e = c.apow_C; e > 0; e >>= 1) {
+                    if (e & 1) { const double r = pr * br - pi * bi, q = pr * bi + pi * br; pr = r; pi = q; }
+                    const double r = br * br - bi * bi, q = 2.0 * br * bi; br = r; bi = q;
+                }
+                apow[2 * i] = (float)pr; apow[2 * i + 1] = (float)pi;
+            }
+            SPIIR_TRY(cudaMemcpy(c.d_apow, apow.data(), c.nfilt * sizeof(float2), cudaMemcpyHostToDevice));
+        }
         if (c.d_tmap) SPIIR_TRY(cudaMemcpy(c.d_tmap, members[ci].data(), (size_t)c.T * sizeof(int32_t), cudaMemcpyHostToDevice));
         if (c.d_chunk) SPIIR_TRY(cudaMemset(c.d_chunk, 0, (size_t)c.NC_cap * p->S * c.nfilt * sizeof(float2)));
     }

@@ -33,6 +33,7 @@ constexpr int kMaxWarps = 8;      // warps per CTA (launch bound 256 threads -> 
 struct FilterArgs {
     const float4* coef;      // [G][F][32]  (a1.re, a1.im, b0.re, b0.im), plan order
     const int*    dly;       // [G][F][32]  delay in samples
+    const float2* apow;      // [G][F][32]  a1^C for this launch's chunk length C (in-CTA scan), or nullptr: computed in the kernel
     float2*       state;     // [S][sstride], this bank's [G][F][32] carried y (in/out) at the start of every row
     size_t        sstride;   // elements between the state rows of two streams
     float2*       chunk_st;  // chunked modes: [S][NC][G][F][32]; pass 1 writes end states, carry
@@ -538,12 +539,13 @@ __global__ void __launch_bounds__(kScanMaxWarps * 32) spiir_filter_scan_kernel(c
     float2* st = a.state + (size_t)s * a.sstride + lbase;
 
     // coefficient / delay / state loads first: their DRAM round trip overlaps the one of the phase word and the window
-    float4 cf[F]; float2 Y[F], aC[F]; int off4[F], dl[F];
+    float4 cf[F]; float2 Y[F], Y0[F], aC[F]; int off4[F], dl[F];
 #pragma unroll
     for (int f = 0; f < F; ++f) {
         cf[f] = a.coef[lbase + (size_t)f * 32];
         dl[f] = a.dly[lbase + (size_t)f * 32];
         Y[f] = (c == 0) ? st[(size_t)f * 32] : make_float2(0.f, 0.f);
+        if (a.apow) aC[f] = a.apow[lbase + (size_t)f * 32];           // a1^C from the plan's table (same chunk length)
     }
     const int ph = phase_parity(a.phase);
     if (a.carry && threadIdx.x == 0) phase_arrive(a.phase, blockIdx.y * gridDim.x + blockIdx.x, gridDim.x * gridDim.y);
@@ -557,13 +559,16 @@ __global__ void __launch_bounds__(kScanMaxWarps * 32) spiir_filter_scan_kernel(c
         const int d = dl[f];
         const int sh = (-d) & 3;
         off4[f] = (sh * a.CS + a.Dpad - d - sh) >> 2;
-        // a1^C, C = chunk length, by repeated squaring in double
-        double pr = 1.0, pi = 0.0, br = (double)cf[f].x, bi = (double)cf[f].y;
-        for (int e = a.C; e > 0; e >>= 1) {
-            if (e & 1) { const double r = pr * br - pi * bi, q = pr * bi + pi * br; pr = r; pi = q; }
-            const double r = br * br - bi * bi, q = 2.0 * br * bi; br = r; bi = q;
+        if (!a.apow) {
+            // a1^C, C = chunk length, by repeated squaring in double (1 us for a 512-thread CTA: only for block lengths
+            // the plan holds no table for)
+            double pr = 1.0, pi = 0.0, br = (double)cf[f].x, bi = (double)cf[f].y;
+            for (int e = a.C; e > 0; e >>= 1) {
+                if (e & 1) { const double r = pr * br - pi * bi, q = pr * bi + pi * br; pr = r; pi = q; }
+                const double r = br * br - bi * bi, q = 2.0 * br * bi; br = r; bi = q;
+            }
+            aC[f] = make_float2((float)pr, (float)pi);
         }
-        aC[f] = make_float2((float)pr, (float)pi);
     }
     const float4* win4 = reinterpret_cast<const float4*>(win);
     const int ntiles = (a.n + a.NT - 1) / a.NT;
@@ -579,32 +584,42 @@ __global__ void __launch_bounds__(kScanMaxWarps * 32) spiir_filter_scan_kernel(c
         }
         const int nch = (len + a.C - 1) / a.C;
         const int cbeg = c * a.C, clen = min(a.C, len - cbeg);
+        // Phase 1: every chunk but the last runs WITHOUT output to find its end state -- chunk 0 from the true state
+        // (so its end is true), the others from zero.  Chunk 0 does not emit yet either: its pass with output is 2x
+        // the cost of a pass without, and every other warp would wait for it at the barrier.
         if (c == 0) {
             if (tile > 0) {
 #pragma unroll
                 for (int f = 0; f < F; ++f) Y[f] = ex[f * 32 + lane];
             }
-            scan_run_chunk<F, LPT, false>(win4, off4, cf, Y, t0, 0, clen, lane, oc);
 #pragma unroll
-            for (int f = 0; f < F; ++f) ex[((nch > 1 ? 1 : 0) * F + f) * 32 + lane] = Y[f];
-        } else if (c < nch - 1) {
+            for (int f = 0; f < F; ++f) Y0[f] = Y[f];
+        }
+        if (c < nch - 1) {
+            if (c > 0) {
 #pragma unroll
-            for (int f = 0; f < F; ++f) Y[f] = make_float2(0.f, 0.f);
+                for (int f = 0; f < F; ++f) Y[f] = make_float2(0.f, 0.f);
+            }
             scan_run_chunk<F, LPT, true>(win4, off4, cf, Y, t0, cbeg, clen, lane, oc);
 #pragma unroll
             for (int f = 0; f < F; ++f) ex[((c + 1) * F + f) * 32 + lane] = Y[f];
         }
         __syncthreads();
-        if (c >= 1 && c < nch) {
+        // Phase 2: true initial state of every chunk (ex[1] = true end of chunk 0, then y <- a1^C y + zero-state end),
+        // and the pass that emits z.
+        if (c < nch) {
 #pragma unroll
             for (int f = 0; f < F; ++f) {
-                float2 v = ex[(F + f) * 32 + lane];                    // true end of chunk 0 = initial state of chunk 1
-                for (int j = 1; j < c; ++j) {
-                    const float2 e = ex[((j + 1) * F + f) * 32 + lane];
-                    float2 nx;
-                    nx.x = fmaf(aC[f].x, v.x, fmaf(-aC[f].y, v.y, e.x));
-                    nx.y = fmaf(aC[f].x, v.y, fmaf(aC[f].y, v.x, e.y));
-                    v = nx;
+                float2 v = Y0[f];
+                if (c >= 1) {
+                    v = ex[(F + f) * 32 + lane];
+                    for (int j = 1; j < c; ++j) {
+                        const float2 e = ex[((j + 1) * F + f) * 32 + lane];
+                        float2 nx;
+                        nx.x = fmaf(aC[f].x, v.x, fmaf(-aC[f].y, v.y, e.x));
+                        nx.y = fmaf(aC[f].x, v.y, fmaf(aC[f].y, v.x, e.y));
+                        v = nx;
+                    }
                 }
                 Y[f] = v;
             }

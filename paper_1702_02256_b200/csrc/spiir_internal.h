@@ -88,6 +88,8 @@ struct spiir_bank_class {
     size_t state_off = 0;             // offset of the class inside a stream's state row (elements)
     int NC_cap = 1;                   // chunk scratch is sized for this many chunks
     float4* d_coef = nullptr;
+    float2* d_apow = nullptr;         // a1^apow_C in d_coef's order: the in-CTA scan's chunk carry factor at n = max_block
+    int apow_C = 0;
     int32_t* d_dly = nullptr;
     float2* d_chunk = nullptr;
     int32_t* d_tmap = nullptr;        // class template -> output row (nullptr for a uniform bank)
