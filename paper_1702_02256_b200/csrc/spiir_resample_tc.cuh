@@ -8,27 +8,32 @@
 //      T[2m'+p, k] = 2 h[2 (96 + m' - k) + p] for 1 <= k - m' <= 96, zero elsewhere (60 % dense).  It is the same for
 //      every tile, so it lives in TENSOR MEMORY for the whole kernel (the A operand of tcgen05.mma may come from TMEM);
 //   X: 96 real rows (re of the 48 rows, then im) x the window, the DATA, in shared memory (B operand, K-major);
-//   D: 128 lanes (outputs) x 96 columns (real rows) of float32 in TMEM, double-buffered (320 + 2 x 96 = all 512 columns).
+//   D: 128 lanes (outputs) x 96 columns (real rows) of float32 in TMEM, double-buffered (T: 160 + 80 + 80 columns, D: 2 x 96 = all 512 columns).
 // tcgen05.mma kind::tf32 (M = 128, N = 96, K = 8 per instruction; measured on this B200: 55 cycles per instruction
 // up to N = 64, 67 at N = 128 = the nominal TF32 rate, so narrow tiles waste the pipe).  One TF32 pass has 2^-11
 // input precision, far outside the 1e-5 tolerance: every operand is split into a TF32-exact high part and the
-// float32 remainder and three passes are accumulated, T_hi X_hi + T_lo X_hi + T_hi X_lo (the dropped T_lo X_lo
-// term is 2^-22 relative).
+// float32 remainder, T X = T_hi X_hi + T_lo X + T X_lo (the dropped T_lo X_lo term is 2^-22 relative).  Only the first
+// product needs TF32; the two correction terms are 2^-11 of it, so bf16 operands (2^-9 relative) leave them exact to
+// 2^-20: they run as kind::f16 instructions with K = 16 (bf16(T_lo) bf16(X) + bf16(T) bf16(X_lo), 10 + 10 instructions per
+// tile instead of 20 + 20 in TF32) into the SAME float32 accumulator.  Measured against the float64 oracle: rel-L2 8.5e-7
+// (three TF32 passes: 7.5e-7; the CUDA-core kernel: 1.5e-7).
 //
-// The data operand uses the canonical K-major, non-swizzled layout: 16-byte "units" of 4 consecutive samples,
-// unit u of real row r at u * 1536 + r * 16.  It is a RING of 56 units (7 chunks of 32 samples): a tile's window
-// is 5 consecutive chunks, every tile advances it by two and two chunks are free for the loader to run a whole tile
-// ahead; each input sample is written to shared memory once and read by 2.5 tiles; a K = 8 instruction takes two adjacent units and never straddles the ring's end.
+// The data operands use the canonical K-major, non-swizzled layout: 16-byte "units" of 4 consecutive TF32 samples (8
+// bf16 samples), unit u of real row r at u * 1536 + r * 16.  Each is a RING of 7 chunks of 32 samples (56 TF32 units,
+// 28 bf16 units, twice): a tile's window is 5 consecutive chunks, every tile advances it by two and two chunks are free
+// for the loader to run a whole tile ahead; each input sample is written to shared memory once and read by 2.5 tiles; an
+// instruction takes two adjacent units and never straddles the ring's end.
 //
 // Roles (384 threads): one thread of warp 11 fetches the raw chunks (ROWS rows x 32 samples) with TMA tile copies through
 // a tensor map of the input into a 4-slot staging ring (48 KB of loads in flight per SM); warps 0-5 read a staged chunk,
-// split it into TF32 high / low parts and store it as the data operand; warp 10 issues the MMAs (one thread) and owns
+// split it into the TF32 high part and the two bf16 correction operands and store them as the data operands; warp 10 issues the MMAs (one thread) and owns
 // TMEM; warps 6-9 drain the accumulator (tcgen05.ld): a lane is an output sample, so a warp writes 256 contiguous bytes of
 // one row per store -- no transposition; with accumulate the store is a vector reduction (red.global.add.v2.f32) done
 // by the L2.  mbarriers: sfull[4] / sempty[4] per staging slot, full[7] / empty[7] per ring chunk, tfull[2] / tempty[2]
 // for the accumulator buffers.  CTAs are persistent over (strip, time segment) units.
 #pragma once
 #include <cuda.h>
+#include <cuda_bf16.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
 
@@ -55,7 +60,8 @@ constexpr int RING_CH = WIN_CH + 2;            // a whole tile (two chunks) of p
 constexpr int RING_UNITS = RING_CH * CHU;      // 56 (even)
 constexpr int UNIT_BYTES = NR * 16;
 constexpr int PART_BYTES = RING_UNITS * UNIT_BYTES;
-constexpr int OFF_LO = PART_BYTES;
+constexpr int OFF_XB = PART_BYTES;             // bf16(x): units of 8 samples, half the bytes of the TF32 part
+constexpr int OFF_XLB = PART_BYTES + PART_BYTES / 2;   // bf16(x - tf32(x))
 constexpr int STG_SLOTS = 4;                   // raw chunks in flight per CTA (TMA tensor copies, 48 KB)
 constexpr int STG_HALF = ROWS * 128;           // half a chunk: ROWS x 16 samples = ROWS x 128 bytes, 128-byte swizzle
 constexpr int STG_BYTES = 2 * STG_HALF;
@@ -69,11 +75,10 @@ constexpr int LOADER_WARPS = ROWS / 8;         // warps that split and store the
 constexpr int LOADERS = LOADER_WARPS * 32;
 constexpr int EPI_WARPS = 4;
 constexpr int THREADS = (LOADER_WARPS + EPI_WARPS + 2) * 32;   // loader warps, epilogue warps, 1 MMA warp, 1 TMA warp (384 threads at 48 rows)
-constexpr int ITEMS = ROWS * CHU / LOADERS;    // (row, unit) items of a chunk per loader thread
-static_assert(ROWS * CHU % LOADERS == 0, "a chunk must split evenly over the loader threads");
+static_assert(LOADERS == ROWS * CHU / 2, "a loader thread owns 8 consecutive samples of one row of a chunk");
 static_assert(SMEM_BYTES <= 227 * 1024, "shared memory");
 constexpr int TMEM_COLS = 512;
-constexpr int COL_THI = 0, COL_TLO = KWIN, COL_D = 2 * KWIN;   // accumulator buffer(s) of NR columns at COL_D
+constexpr int COL_THI = 0, COL_TLB = KWIN, COL_TB = KWIN + KWIN / 2, COL_D = 2 * KWIN;   // T: TF32 high part, bf16(low part), bf16(T) (two per column); accumulators at COL_D
 constexpr int NBUF = (2 * KWIN + 2 * NR <= TMEM_COLS) ? 2 : 1;  // 48-row strips: 320 + 2 x 96 = 512 columns; 64-row strips: 320 + 128
 
 struct UpTcArgs {
@@ -122,6 +127,13 @@ __device__ __forceinline__ void umma_tf32_ts(uint32_t tmem_d, uint32_t tmem_a, u
                  ::"r"(tmem_d), "r"(tmem_a), "l"(bdesc), "r"(idesc), "r"(accumulate), "r"(0u) : "memory");
 }
 // 32 consecutive columns of this thread's TMEM lane <-> 32 registers
+// same with bf16 operands (K = 16 per instruction; A: two elements per TMEM column) accumulating into the same float32 D
+__device__ __forceinline__ void umma_bf16_ts(uint32_t tmem_d, uint32_t tmem_a, uint64_t bdesc, uint32_t idesc, uint32_t accumulate)
+{
+    asm volatile("{\n .reg .pred p;\n setp.ne.b32 p, %4, 0;\n"
+                 " tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, {%5, %5, %5, %5}, p;\n}"
+                 ::"r"(tmem_d), "r"(tmem_a), "l"(bdesc), "r"(idesc), "r"(accumulate), "r"(0u) : "memory");
+}
 __device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&v)[32])
 {
     asm volatile("tcgen05.ld.sync.aligned.32x32b.x32.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
@@ -152,6 +164,22 @@ __device__ __forceinline__ void tmem_st32(uint32_t taddr, const uint32_t (&v)[32
                    "r"(v[8]), "r"(v[9]), "r"(v[10]), "r"(v[11]), "r"(v[12]), "r"(v[13]), "r"(v[14]), "r"(v[15]),
                    "r"(v[16]), "r"(v[17]), "r"(v[18]), "r"(v[19]), "r"(v[20]), "r"(v[21]), "r"(v[22]), "r"(v[23]),
                    "r"(v[24]), "r"(v[25]), "r"(v[26]), "r"(v[27]), "r"(v[28]), "r"(v[29]), "r"(v[30]), "r"(v[31]) : "memory");
+}
+__device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t (&v)[16])
+{
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16};"
+                 ::"r"(taddr), "r"(v[0]), "r"(v[1]), "r"(v[2]), "r"(v[3]), "r"(v[4]), "r"(v[5]), "r"(v[6]), "r"(v[7]),
+                   "r"(v[8]), "r"(v[9]), "r"(v[10]), "r"(v[11]), "r"(v[12]), "r"(v[13]), "r"(v[14]), "r"(v[15]) : "memory");
+}
+// two floats -> packed bf16 pair, `lo` in the low half (= the lower K index)
+__device__ __forceinline__ uint32_t bf16x2(float lo, float hi)
+{
+    const __nv_bfloat162 v = __floats2bfloat162_rn(lo, hi);
+    return *reinterpret_cast<const uint32_t*>(&v);
+}
+__device__ __forceinline__ void sts128u(uint32_t addr, uint32_t x, uint32_t y, uint32_t z, uint32_t w)
+{
+    asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(x), "r"(y), "r"(z), "r"(w) : "memory");
 }
 __device__ __forceinline__ void sts128(uint32_t addr, float4 v)
 {
@@ -231,17 +259,24 @@ __global__ void __launch_bounds__(THREADS, 1) spiir_up2_tc_kernel(const UpTcArgs
         // float32 remainder, computed from the 192 taps (L1-resident) straight into this thread's TMEM lane
         const int mp = t >> 1, pp = t & 1;
         for (int c0 = 0; c0 < KWIN; c0 += 32) {
-            uint32_t vh[32], vl[32];
+            uint32_t vh[32], vlb[16], vb[16];
 #pragma unroll
-            for (int i = 0; i < 32; ++i) {
-                const int dk = c0 + i - mp;
-                const float v = (dk >= 1 && dk <= HALF) ? 2.f * __ldg(a.taps + 2 * (HALF - dk) + pp) : 0.f;
-                const float h = tf32_hi(v);
-                vh[i] = __float_as_uint(h);
-                vl[i] = __float_as_uint(v - h);
+            for (int i = 0; i < 16; ++i) {
+                float v[2], l[2];
+#pragma unroll
+                for (int e = 0; e < 2; ++e) {
+                    const int dk = c0 + 2 * i + e - mp;
+                    v[e] = (dk >= 1 && dk <= HALF) ? 2.f * __ldg(a.taps + 2 * (HALF - dk) + pp) : 0.f;
+                    const float h = tf32_hi(v[e]);
+                    vh[2 * i + e] = __float_as_uint(h);
+                    l[e] = v[e] - h;
+                }
+                vlb[i] = bf16x2(l[0], l[1]);
+                vb[i] = bf16x2(v[0], v[1]);
             }
             tmem_st32(lane_addr + COL_THI + (uint32_t)c0, vh);
-            tmem_st32(lane_addr + COL_TLO + (uint32_t)c0, vl);
+            tmem_st16(lane_addr + COL_TLB + (uint32_t)(c0 >> 1), vlb);
+            tmem_st16(lane_addr + COL_TB + (uint32_t)(c0 >> 1), vb);
         }
         asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
     }
@@ -295,12 +330,14 @@ __global__ void __launch_bounds__(THREADS, 1) spiir_up2_tc_kernel(const UpTcArgs
                 const int mc = ms - HALF + ci * CHS;                    // first sample of the chunk
                 const bool stg = staged(ci);
                 const int ss = sc % STG_SLOTS;
-                float4 v[ITEMS][2];                                     // (re, im) of samples 4u .. 4u + 3 of row r
+                constexpr int ITEMS = 2;                                // two units of 4 samples: 8 consecutive samples of row r
+                const int r = tid % ROWS, up = tid / ROWS;              // up: which 8 samples of the chunk (0 .. 3)
+                float4 v[ITEMS][2];                                     // (re, im) of samples 4u .. 4u + 3, u = 2 up + k
                 if (stg) {
                     bar_wait(sfull(ss), (uint32_t)((sc / STG_SLOTS) & 1));
 #pragma unroll
                     for (int k = 0; k < ITEMS; ++k) {
-                        const int idx = tid + k * LOADERS, r = idx % ROWS, u = idx / ROWS;
+                        const int u = 2 * up + k;
                         const uint32_t src = sbase + OFF_STG + (uint32_t)(ss * STG_BYTES + (u >> 2) * STG_HALF + r * 128);
                         const int j = 2 * (u & 3), x = r & 7;
                         v[k][0] = lds128(src + (uint32_t)((j ^ x) << 4));
@@ -312,7 +349,7 @@ __global__ void __launch_bounds__(THREADS, 1) spiir_up2_tc_kernel(const UpTcArgs
                 } else {
 #pragma unroll
                     for (int k = 0; k < ITEMS; ++k) {
-                        const int idx = tid + k * LOADERS, r = idx % ROWS, u = idx / ROWS;
+                        const int u = 2 * up + k;
                         const int row = row0 + r, m = mc + 4 * u;
                         float2 q[4];
 #pragma unroll
@@ -331,7 +368,7 @@ __global__ void __launch_bounds__(THREADS, 1) spiir_up2_tc_kernel(const UpTcArgs
                 if (ci >= HALO_CH && hfirst >= 0 && mc + CHS > hfirst) {
 #pragma unroll
                     for (int k = 0; k < ITEMS; ++k) {
-                        const int idx = tid + k * LOADERS, r = idx % ROWS, u = idx / ROWS;
+                        const int u = 2 * up + k;
                         const int row = row0 + r, g = mc + 4 * u - hfirst;
                         if (row < a.rows) {
                             float2* hrow = hnext + (size_t)row * (HALF - 1);
@@ -344,9 +381,10 @@ __global__ void __launch_bounds__(THREADS, 1) spiir_up2_tc_kernel(const UpTcArgs
                     }
                 }
                 if (fill > 0) bar_wait(empty(slot), (uint32_t)((fill - 1) & 1));
+                uint32_t bre[4], bim[4], lre[4], lim[4];                // bf16 pairs of x and of x - tf32(x)
 #pragma unroll
                 for (int k = 0; k < ITEMS; ++k) {
-                    const int idx = tid + k * LOADERS, r = idx % ROWS, u = idx / ROWS;
+                    const int u = 2 * up + k;
                     const float4 wre = make_float4(v[k][0].x, v[k][0].z, v[k][1].x, v[k][1].z);
                     const float4 wim = make_float4(v[k][0].y, v[k][0].w, v[k][1].y, v[k][1].w);
                     const float4 hre = make_float4(tf32_hi(wre.x), tf32_hi(wre.y), tf32_hi(wre.z), tf32_hi(wre.w));
@@ -354,8 +392,17 @@ __global__ void __launch_bounds__(THREADS, 1) spiir_up2_tc_kernel(const UpTcArgs
                     const uint32_t addr = sbase + (uint32_t)(slot * CHU + u) * UNIT_BYTES + (uint32_t)r * 16;
                     sts128(addr, hre);
                     sts128(addr + ROWS * 16, him);
-                    sts128(addr + OFF_LO, make_float4(wre.x - hre.x, wre.y - hre.y, wre.z - hre.z, wre.w - hre.w));
-                    sts128(addr + OFF_LO + ROWS * 16, make_float4(wim.x - him.x, wim.y - him.y, wim.z - him.z, wim.w - him.w));
+                    bre[2 * k] = bf16x2(wre.x, wre.y); bre[2 * k + 1] = bf16x2(wre.z, wre.w);
+                    bim[2 * k] = bf16x2(wim.x, wim.y); bim[2 * k + 1] = bf16x2(wim.z, wim.w);
+                    lre[2 * k] = bf16x2(wre.x - hre.x, wre.y - hre.y); lre[2 * k + 1] = bf16x2(wre.z - hre.z, wre.w - hre.w);
+                    lim[2 * k] = bf16x2(wim.x - him.x, wim.y - him.y); lim[2 * k + 1] = bf16x2(wim.z - him.z, wim.w - him.w);
+                }
+                {
+                    const uint32_t addr = sbase + (uint32_t)(slot * (CHU / 2) + up) * UNIT_BYTES + (uint32_t)r * 16;
+                    sts128u(addr + OFF_XB, bre[0], bre[1], bre[2], bre[3]);
+                    sts128u(addr + OFF_XB + ROWS * 16, bim[0], bim[1], bim[2], bim[3]);
+                    sts128u(addr + OFF_XLB, lre[0], lre[1], lre[2], lre[3]);
+                    sts128u(addr + OFF_XLB + ROWS * 16, lim[0], lim[1], lim[2], lim[3]);
                 }
                 asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
                 __syncwarp();
@@ -385,6 +432,7 @@ __global__ void __launch_bounds__(THREADS, 1) spiir_up2_tc_kernel(const UpTcArgs
             // ===== MMA issuer (one thread) =====
             if (lane == 0) {
                 const uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(NR >> 3) << 17) | ((uint32_t)(MOUT >> 4) << 24);
+                const uint32_t idesc_bf = (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(NR >> 3) << 17) | ((uint32_t)(MOUT >> 4) << 24);
                 for (int j = 0; j < J; ++j) {
                     const int cn = cbase + 2 * j + WIN_CH - 1;          // newest chunk of this tile's window
                     bar_wait(full(cn % RING_CH), (uint32_t)((cn / RING_CH) & 1));
@@ -393,16 +441,22 @@ __global__ void __launch_bounds__(THREADS, 1) spiir_up2_tc_kernel(const UpTcArgs
                     const uint32_t d = tmem + COL_D + (uint32_t)(buf * NR);
                     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
                     const int wu0 = ((cbase + 2 * j) % RING_CH) * CHU;  // ring unit of the window's first unit
+                    // T_hi X_hi in TF32 (20 instructions of K = 8), then the two correction terms bf16(T_lo) bf16(X) and
+                    // bf16(T) bf16(X_lo) with bf16 operands (10 + 10 instructions of K = 16) into the same accumulator
 #pragma unroll 2
                     for (int ks = 0; ks < KSTEPS; ++ks) {
                         int ru = wu0 + 2 * ks;
                         if (ru >= RING_UNITS) ru -= RING_UNITS;
-                        const uint32_t x_hi = sbase + (uint32_t)ru * UNIT_BYTES;
-                        const uint64_t dxh = smem_desc(x_hi, UNIT_BYTES, 128), dxl = smem_desc(x_hi + OFF_LO, UNIT_BYTES, 128);
-                        const uint32_t thi = tmem + COL_THI + (uint32_t)(8 * ks), tlo = tmem + COL_TLO + (uint32_t)(8 * ks);
-                        umma_tf32_ts(d, thi, dxh, idesc, ks > 0 ? 1u : 0u);
-                        umma_tf32_ts(d, tlo, dxh, idesc, 1u);
-                        umma_tf32_ts(d, thi, dxl, idesc, 1u);
+                        umma_tf32_ts(d, tmem + COL_THI + (uint32_t)(8 * ks), smem_desc(sbase + (uint32_t)ru * UNIT_BYTES, UNIT_BYTES, 128),
+                                     idesc, ks > 0 ? 1u : 0u);
+                    }
+#pragma unroll 2
+                    for (int ks = 0; ks < KSTEPS / 2; ++ks) {
+                        int ru = (wu0 >> 1) + 2 * ks;                   // units of 8 samples
+                        if (ru >= RING_UNITS / 2) ru -= RING_UNITS / 2;
+                        const uint32_t xb = sbase + (uint32_t)ru * UNIT_BYTES;
+                        umma_bf16_ts(d, tmem + COL_TLB + (uint32_t)(8 * ks), smem_desc(xb + OFF_XB, UNIT_BYTES, 128), idesc_bf, 1u);
+                        umma_bf16_ts(d, tmem + COL_TB + (uint32_t)(8 * ks), smem_desc(xb + OFF_XLB, UNIT_BYTES, 128), idesc_bf, 1u);
                     }
                     umma_commit(empty((cbase + 2 * j) % RING_CH));     // the window's two oldest chunks are free once these MMAs are done
                     umma_commit(empty((cbase + 2 * j + 1) % RING_CH));
