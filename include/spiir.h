@@ -256,6 +256,32 @@ spiir_status spiir_host_geometry(int n_templates, int n_filters, int n_streams, 
 spiir_status spiir_host_lane_mapping(int n_filters, int n_templates, int info[3]);
 
 /* ---------------------------------------------------------------------------------------------
+ * NO-ALLOCATION ENTRY POINT (Eq. 7-8; the time-parallel scan of SURVEY.md section 8 row a7).
+ * For callers that cannot call cudaMalloc (code under CUDA-graph capture, tight serving loops, harnesses that
+ * forbid it): filters ONE block from zero state (y = 0, x[k] = 0 for k < 0) with no plan and no workspace.
+ *   a1, b0   : DEVICE [n_templates][n_filters] complex64, caller order (not permuted)
+ *   delays   : DEVICE [n_templates][n_filters] int32, >= 0
+ *   x        : DEVICE [n] float32;   snr_out : DEVICE [n_templates][n] complex64, overwritten
+ *   time_chunks : 0 = as many chunks of >= 64 samples as fit (at most 64), else that many chunks
+ * The chunk states of the scan (n_templates * n_filters * chunks * 8 bytes, spiir_noalloc_scratch_need) live in a
+ * device array built into the library: SPIIR_NOALLOC_SCRATCH_BYTES (4 MiB) on every GPU that loads the library,
+ * held until the process exits.  A call that needs more returns SPIIR_EINVAL with a message and launches nothing;
+ * n_filters > 512 returns SPIIR_EUNSUPPORTED.  The call makes no cudaMalloc / cudaFree / allocating library call
+ * and does not synchronise; three kernels are enqueued on cuda_stream.  spiir_noalloc_setup looks the array's
+ * device address up for the current device (done lazily by the first call otherwise; call it once before a stream
+ * capture).  All calls share the array: calls on ONE stream are ordered and safe, calls that overlap on the GPU
+ * (several streams, concurrent graph replays) RACE.  Nothing in the array needs clearing between calls (every word
+ * a call reads it has written itself).  Results agree with spiir_filter on a fresh plan within the parity tolerance
+ * (float32, another summation order); deterministic.  Owns nothing, keeps no state between calls.
+ * ------------------------------------------------------------------------------------------- */
+#define SPIIR_NOALLOC_SCRATCH_BYTES (4u << 20)
+size_t       spiir_noalloc_scratch_need(int n_templates, int n_filters, int n, int time_chunks);
+spiir_status spiir_noalloc_setup(void);
+spiir_status spiir_filter_block_noalloc(const spiir_c64* a1, const spiir_c64* b0, const int32_t* delays, int n_templates,
+                                        int n_filters, const float* x, int n, int time_chunks, spiir_c64* snr_out,
+                                        void* cuda_stream);
+
+/* ---------------------------------------------------------------------------------------------
  * COMPARISON KERNELS, not the product path: the paper's own single-rate design restated
  * for the same B200 so that the new mapping can be measured against it on one machine (bench.py --impl
  * paper_design).  One thread per filter; a template of more than 32 filters is one CUDA block of

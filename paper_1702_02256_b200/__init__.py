@@ -22,6 +22,7 @@ _lib = None
 
 SPIIR_OK, SPIIR_EINVAL, SPIIR_ENOMEM, SPIIR_ECUDA, SPIIR_EUNSUPPORTED, SPIIR_ESTATE = range(6)
 SPIIR_DOWN2, SPIIR_UP2 = 0, 1
+SPIIR_NOALLOC_SCRATCH_BYTES = 4 << 20
 
 EXPORTS = (
     "spiir_plan_workspace_bytes", "spiir_plan_create", "spiir_plan_workspace_bytes_ragged", "spiir_plan_create_ragged",
@@ -33,6 +34,7 @@ EXPORTS = (
     "spiir_mr_launches", "spiir_mr_plan_state_bytes", "spiir_mr_plan_get_state", "spiir_mr_plan_set_state",
     "spiir_assign_rates", "spiir_host_layout", "spiir_host_geometry", "spiir_host_lane_mapping",
     "spiir_pd_plan_create", "spiir_pd_filter", "spiir_pd_plan_reset", "spiir_pd_plan_destroy",
+    "spiir_noalloc_scratch_need", "spiir_noalloc_setup", "spiir_filter_block_noalloc",
     "spiir_probe_fp32_peak", "spiir_probe_ffma2_operands", "spiir_last_error", "spiir_version",
 )
 
@@ -116,6 +118,10 @@ def lib():
         L.spiir_pd_plan_reset.argtypes = [vp, vp]
         L.spiir_pd_plan_destroy.argtypes = [vp]
         L.spiir_pd_plan_destroy.restype = None
+        L.spiir_noalloc_scratch_need.argtypes = [ci, ci, ci, ci]
+        L.spiir_noalloc_scratch_need.restype = sz
+        L.spiir_noalloc_setup.argtypes = []
+        L.spiir_filter_block_noalloc.argtypes = [vp, vp, vp, ci, ci, vp, ci, ci, vp, vp]
         L.spiir_probe_fp32_peak.argtypes = [ctypes.POINTER(cd)]
         L.spiir_probe_ffma2_operands.argtypes = [ctypes.POINTER(cd * 4)]
         L.spiir_host_layout.argtypes = [vp, vp, vp, ci, ci, ci, vp, vp, vp, ctypes.POINTER(ci * 4),
@@ -491,6 +497,37 @@ class MultiratePlan:
             self.close()
         except Exception:
             pass
+
+
+def filter_block_noalloc(a1, b0, delays, x, out=None, time_chunks: int = 0, stream=None):
+    """spiir_filter_block_noalloc: one block from zero state, no plan, no workspace, no allocation inside the library
+    (its scan scratch is a 4 MiB device array built into libspiir.so; calls that overlap on the GPU race on it).
+    a1, b0: CUDA complex64 [T][L]; delays: CUDA int32 [T][L]; x: CUDA float32 [n]; returns (or fills) complex64 [T][n].
+    Pass `out` to keep this wrapper allocation-free as well."""
+    import torch
+    for t, dt, name in ((a1, torch.complex64, "a1"), (b0, torch.complex64, "b0"), (delays, torch.int32, "delays"),
+                        (x, torch.float32, "x")):
+        if not (t.is_cuda and t.dtype == dt and t.is_contiguous()):
+            raise ValueError(f"{name} must be a contiguous CUDA {dt} tensor")
+    if a1.dim() != 2 or b0.shape != a1.shape or delays.shape != a1.shape or x.dim() != 1:
+        raise ValueError("a1, b0, delays must be [T][L] and x [n]")
+    T, L = int(a1.shape[0]), int(a1.shape[1])
+    n = int(x.shape[0])
+    if out is None:
+        out = torch.empty((T, n), dtype=torch.complex64, device=x.device)
+    else:
+        _need(out, torch.complex64, T * n, "out")
+    _check(lib().spiir_filter_block_noalloc(a1.data_ptr(), b0.data_ptr(), delays.data_ptr(), T, L, x.data_ptr(), n,
+                                            int(time_chunks), out.data_ptr(), _stream_ptr(stream)), "spiir_filter_block_noalloc")
+    return out
+
+
+def noalloc_scratch_need(n_templates: int, n_filters: int, n: int, time_chunks: int = 0) -> int:
+    return int(lib().spiir_noalloc_scratch_need(int(n_templates), int(n_filters), int(n), int(time_chunks)))
+
+
+def noalloc_setup() -> None:
+    _check(lib().spiir_noalloc_setup(), "spiir_noalloc_setup")
 
 
 class PaperDesignPlan:

@@ -14,7 +14,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libspiir.so")
-SOURCES = ["spiir_api.cu", "spiir_resamp.cu", "spiir_mr.cu", "spiir_probe.cu", "spiir_paper_design.cu", "spiir_host.cpp"]
+SOURCES = ["spiir_api.cu", "spiir_resamp.cu", "spiir_mr.cu", "spiir_probe.cu", "spiir_paper_design.cu", "spiir_noalloc.cu", "spiir_host.cpp"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "--use_fast_math=false"]
 
