@@ -424,7 +424,7 @@ def resample_leg(sp, timer, direction: str, taps: int, rows: int, steps: int, wa
                         "bytes_per_output": bytes_per_out},
            "roofline_alu": {"bound": "alu", "achieved": n_out * fma_per_out * 2 / t / 1e12, "peak": 2 * fma_peak / 1e12,
                             "unit": "TFLOP/s", "frac": n_out * fma_per_out / t / fma_peak, "fma_per_output": fma_per_out}}
-    if up and taps == 192:
+    if up and taps in (192, 32):
         # this stage runs on the tensor cores (spiir_up2_tc_kernel): the FP32 figure is the CUDA-core rate the same useful
         # arithmetic would need, a fraction above 1 means CUDA cores could not do it in this time
         leg["roofline_alu"]["note"] = ("executed by tcgen05.mma (TF32 + two bf16 correction products), not by FP32 FMAs: "

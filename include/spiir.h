@@ -155,7 +155,7 @@ spiir_status spiir_kaiser_taps(int n_taps, double kaiser_beta, double cutoff, fl
  *   n_taps even, 2 <= n_taps <= 1024; taps are spiir_kaiser_taps(n_taps, kaiser_beta, cutoff).
  *   Register-blocked kernels exist for 384 / 192 / 32 taps (the paper's 384-tap
  *   down and 32-tap up filters; configs[3]: 192), a generic kernel serves every other count.
- *   The 192-tap up stage of a large call (rows * n_in >= 65536) runs on the tensor cores: the polyphase FIR as
+ *   The 192-tap and the 32-tap up stage of a large call (rows * n_in >= 65536) run on the tensor cores: the polyphase FIR as
  *   a banded-Toeplitz contraction, tcgen05 kind::tf32 with every operand split into a TF32-exact high part and
  *   its float32 remainder; the product of the high parts and two bf16 correction products accumulate in TMEM
  *   (rel-L2 8.5e-7 against the float64 oracle).  The input is fetched through a tensor map that is
@@ -166,7 +166,7 @@ typedef struct {
     int    max_block;        /* largest n_in of a call */
     void*  workspace;        /* DEVICE, caller-owned; NULL: the library allocates */
     size_t workspace_bytes;
-    int    flags;            /* bit 0: never use the tensor-core kernel (192-tap up stage), for A/B measurements */
+    int    flags;            /* bit 0: never use the tensor-core kernel (192 / 32-tap up stage), for A/B measurements */
 } spiir_resamp_opts;
 
 size_t       spiir_resamp_workspace_bytes(int direction, int n_taps, int n_rows);

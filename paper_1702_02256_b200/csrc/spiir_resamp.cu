@@ -257,20 +257,10 @@ spiir_status spiir_resample_up(spiir_resamp_t* r, const spiir_c64* in, int n_in,
     u.hbuf[0] = reinterpret_cast<float2*>(r->d_hist[0]); u.hbuf[1] = reinterpret_cast<float2*>(r->d_hist[1]);
     u.phase = r->d_phase;
     u.rows = r->rows; u.n_in = n_in; u.accumulate = accumulate;
-    // short filter: HBM-bound streaming kernel, no shared memory.  Its 16-byte input loads need 16-byte aligned rows
-    // (in aligned and n_in even); other inputs take the register-blocked kernel below, which loads 8 bytes at a time.
-    if (r->N == 32 && (reinterpret_cast<uintptr_t>(in) & 15u) == 0 && (n_in & 1) == 0) {
-        u.seg = u.nseg = u.upr = u.rpc = 0;
-        const long long units = (long long)r->rows * ((n_in + kUpSR - 1) / kUpSR);
-        UpTaps<16> t;
-        fill_up_taps<16>(r, &t);
-        spiir_up2_stream_kernel<16><<<(unsigned)((units + 255) / 256), 256, 0, st>>>(u, t);
-        SPIIR_CUDA(cudaGetLastError());
-        return SPIIR_OK;
-    }
-    // 192 taps on the tensor cores (tcgen05 kind::tf32, three-pass split): FP32-bound on the CUDA cores, HBM-bound here.
-    // Needs enough work to fill the persistent CTAs; small calls keep the register-blocked kernel.
-    if (r->N == 2 * tc::HALF && !(r->flags & 1) && (long long)r->rows * n_in >= 64LL * 1024) {
+    // 192 and 32 taps on the tensor cores (tcgen05: TF32 product + two bf16 correction products): FP32-bound (192) or
+    // L1-bound (32) on the CUDA cores, HBM-bound here.  Needs enough work to fill the persistent CTAs; small calls keep
+    // the CUDA-core kernels.
+    if ((r->N == 192 || r->N == 32) && !(r->flags & 1) && (long long)r->rows * n_in >= 64LL * 1024) {
         tc::UpTcArgs t;
         t.in = u.in; t.out = u.out; t.hbuf[0] = u.hbuf[0]; t.hbuf[1] = u.hbuf[1]; t.phase = u.phase; t.taps = r->d_taps;
         t.rows = r->rows; t.n_in = n_in; t.accumulate = accumulate;
@@ -289,8 +279,24 @@ spiir_status spiir_resample_up(spiir_resamp_t* r, const spiir_c64* in, int n_in,
             if (mrc != SPIIR_OK) return mrc;
         }
         const int grid = std::min(t.nstrips * t.nsegs, r->dev.n_sm);
-        SPIIR_CUDA(ensure_smem((const void*)tc::spiir_up2_tc_kernel, tc::SMEM_BYTES));
-        tc::spiir_up2_tc_kernel<<<grid, tc::THREADS, tc::SMEM_BYTES, st>>>(t, in_map);
+        if (r->N == 192) {
+            SPIIR_CUDA(ensure_smem((const void*)tc::spiir_up2_tc_kernel<96, 96>, tc::Geo<96, 96>::SMEM_BYTES));
+            tc::spiir_up2_tc_kernel<96, 96><<<grid, tc::THREADS, tc::Geo<96, 96>::SMEM_BYTES, st>>>(t, in_map);
+        } else {
+            SPIIR_CUDA(ensure_smem((const void*)tc::spiir_up2_tc_kernel<32, 16>, tc::Geo<32, 16>::SMEM_BYTES));
+            tc::spiir_up2_tc_kernel<32, 16><<<grid, tc::THREADS, tc::Geo<32, 16>::SMEM_BYTES, st>>>(t, in_map);
+        }
+        SPIIR_CUDA(cudaGetLastError());
+        return SPIIR_OK;
+    }
+    // short filter: HBM-bound streaming kernel, no shared memory.  Its 16-byte input loads need 16-byte aligned rows
+    // (in aligned and n_in even); other inputs take the register-blocked kernel below, which loads 8 bytes at a time.
+    if (r->N == 32 && (reinterpret_cast<uintptr_t>(in) & 15u) == 0 && (n_in & 1) == 0) {
+        u.seg = u.nseg = u.upr = u.rpc = 0;
+        const long long units = (long long)r->rows * ((n_in + kUpSR - 1) / kUpSR);
+        UpTaps<16> t;
+        fill_up_taps<16>(r, &t);
+        spiir_up2_stream_kernel<16><<<(unsigned)((units + 255) / 256), 256, 0, st>>>(u, t);
         SPIIR_CUDA(cudaGetLastError());
         return SPIIR_OK;
     }

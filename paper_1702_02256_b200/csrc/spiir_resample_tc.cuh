@@ -1,4 +1,4 @@
-// spiir_resample_tc.cuh -- up-by-2 (+ accumulate) with the 192-tap FIR on the 5th-generation tensor cores
+// spiir_resample_tc.cuh -- up-by-2 (+ accumulate) with the 192-tap (or 32-tap) FIR on the 5th-generation tensor cores
 // (row a10 of SURVEY.md section 8; Eq. 9).
 //
 // The polyphase FIR  w[2m+p] = 2 sum_{q<96} h[2q+p] v[m-q]  of a strip of rows is a dense contraction with a banded
@@ -23,6 +23,12 @@
 // 28 bf16 units, twice): a tile's window is 5 consecutive chunks, every tile advances it by two and two chunks are free
 // for the loader to run a whole tile ahead; each input sample is written to shared memory once and read by 2.5 tiles; an
 // instruction takes two adjacent units and never straddles the ring's end.
+//
+// The kernel is a template over (HK, R): R = taps per polyphase branch, HK = the window's halo in whole chunks.  <96, 96> is
+// the 192-tap filter described above; <32, 16> is the paper's own 32-tap up filter run as a 64-tap filter whose
+// outer taps are zero (window of 96 samples, 12 + 6 + 6 instructions per tile): that stage is HBM-bound by its arithmetic,
+// but the CUDA-core streaming kernel was held at 55 % of the HBM peak by L1 wavefronts; here it moves data the same way as
+// the 192-tap stage and runs at the same 84 %.
 //
 // Roles (384 threads): one thread of warp 11 fetches the raw chunks (ROWS rows x 32 samples) with TMA tile copies through
 // a tensor map of the input into a 4-slot staging ring (48 KB of loads in flight per SM); warps 0-5 read a staged chunk,
@@ -49,37 +55,45 @@ constexpr int ROWS = SPIIR_TC_ROWS;            // complex rows per strip: 48 (do
 constexpr int NR = 2 * ROWS;                   // real rows = UMMA N
 constexpr int TIN = 64;                        // input samples per tile
 constexpr int MOUT = 2 * TIN;                  // outputs per tile = UMMA M
-constexpr int HALF = 96;                       // taps per polyphase branch (192-tap filter)
-constexpr int KWIN = HALF + TIN;               // 160
-constexpr int KSTEPS = KWIN / 8;               // 20 MMA k-steps per pass
 constexpr int CHS = 32;                        // samples per chunk
 constexpr int CHU = CHS / 4;                   // units per chunk
-constexpr int WIN_CH = KWIN / CHS;             // 5 chunks per window
-constexpr int HALO_CH = HALF / CHS;            // 3 chunks in front of the first tile of a unit
-constexpr int RING_CH = WIN_CH + 2;            // a whole tile (two chunks) of prefetch space
-constexpr int RING_UNITS = RING_CH * CHU;      // 56 (even)
 constexpr int UNIT_BYTES = NR * 16;
-constexpr int PART_BYTES = RING_UNITS * UNIT_BYTES;
-constexpr int OFF_XB = PART_BYTES;             // bf16(x): units of 8 samples, half the bytes of the TF32 part
-constexpr int OFF_XLB = PART_BYTES + PART_BYTES / 2;   // bf16(x - tf32(x))
 constexpr int STG_SLOTS = 4;                   // raw chunks in flight per CTA (TMA tensor copies, 48 KB)
 constexpr int STG_HALF = ROWS * 128;           // half a chunk: ROWS x 16 samples = ROWS x 128 bytes, 128-byte swizzle
 constexpr int STG_BYTES = 2 * STG_HALF;
-static_assert(STG_HALF % 1024 == 0 && (2 * PART_BYTES) % 1024 == 0, "the 128-byte swizzle pattern repeats every 1024 bytes");
-constexpr int OFF_STG = 2 * PART_BYTES;
-constexpr int OFF_BAR = OFF_STG + STG_SLOTS * STG_BYTES;
-constexpr int NBAR = 2 * RING_CH + 4 + 2 * STG_SLOTS;
-constexpr int OFF_TPTR = OFF_BAR + NBAR * 8;
-constexpr int SMEM_BYTES = OFF_TPTR + 16;
 constexpr int LOADER_WARPS = ROWS / 8;         // warps that split and store the data operand
 constexpr int LOADERS = LOADER_WARPS * 32;
 constexpr int EPI_WARPS = 4;
 constexpr int THREADS = (LOADER_WARPS + EPI_WARPS + 2) * 32;   // loader warps, epilogue warps, 1 MMA warp, 1 TMA warp (384 threads at 48 rows)
 static_assert(LOADERS == ROWS * CHU / 2, "a loader thread owns 8 consecutive samples of one row of a chunk");
-static_assert(SMEM_BYTES <= 227 * 1024, "shared memory");
 constexpr int TMEM_COLS = 512;
-constexpr int COL_THI = 0, COL_TLB = KWIN, COL_TB = KWIN + KWIN / 2, COL_D = 2 * KWIN;   // T: TF32 high part, bf16(low part), bf16(T) (two per column); accumulators at COL_D
-constexpr int NBUF = (2 * KWIN + 2 * NR <= TMEM_COLS) ? 2 : 1;  // 48-row strips: 320 + 2 x 96 = 512 columns; 64-row strips: 320 + 128
+
+// What depends on the filter: R = taps per polyphase branch (96 for the 192-tap filter of configs[3], 16 for the paper's
+// 32-tap up filter), HK >= R = the samples in front of a tile that its window covers, a multiple of the chunk
+// length (96 and 32: the 32-tap filter runs as a 64-tap one whose outer taps are zero).
+template <int HK, int R>
+struct Geo {
+    static_assert(HK % CHS == 0 && R <= HK && R >= 1, "window halo = whole chunks");
+    static constexpr int KWIN = HK + TIN;               // 160 / 96 samples per window
+    static constexpr int KSTEPS = KWIN / 8;             // TF32 k-steps of a tile (bf16: half as many)
+    static constexpr int WIN_CH = KWIN / CHS;           // 5 / 3 chunks per window
+    static constexpr int HALO_CH = HK / CHS;            // chunks in front of the first tile of a unit
+    static constexpr int RING_CH = WIN_CH + 2;          // a whole tile (two chunks) of prefetch space
+    static constexpr int RING_UNITS = RING_CH * CHU;    // even
+    static constexpr int PART_BYTES = RING_UNITS * UNIT_BYTES;
+    static constexpr int OFF_XB = PART_BYTES;           // bf16(x): units of 8 samples, half the bytes of the TF32 part
+    static constexpr int OFF_XLB = PART_BYTES + PART_BYTES / 2;   // bf16(x - tf32(x))
+    static constexpr int OFF_STG = (2 * PART_BYTES + 1023) / 1024 * 1024;   // the 128-byte swizzle pattern repeats every 1024 bytes
+    static constexpr int OFF_BAR = OFF_STG + STG_SLOTS * STG_BYTES;
+    static constexpr int NBAR = 2 * RING_CH + 4 + 2 * STG_SLOTS;
+    static constexpr int OFF_TPTR = OFF_BAR + NBAR * 8;
+    static constexpr int SMEM_BYTES = OFF_TPTR + 16;
+    static_assert(STG_HALF % 1024 == 0 && SMEM_BYTES <= 227 * 1024, "shared memory");
+    // TMEM columns: T as its TF32 high part, bf16(low part), bf16(T) (two per column); accumulator buffer(s) behind
+    static constexpr int COL_THI = 0, COL_TLB = KWIN, COL_TB = KWIN + KWIN / 2, COL_D = 2 * KWIN;
+    static constexpr int NBUF = (2 * KWIN + 2 * NR <= TMEM_COLS) ? 2 : 1;
+    static constexpr int HIST = R - 1;                  // carried history samples per row
+};
 
 struct UpTcArgs {
     const float2* in;        // [rows][n_in]
@@ -213,25 +227,29 @@ __device__ __forceinline__ float tf32_hi(float x)
 }
 
 // sample m of a row (m relative to the block): history for -95 <= m < 0, zero outside
+template <int HIST>
 __device__ __forceinline__ float2 sample_at(const float2* in_row, const float2* hist_row, int m, int n_in)
 {
     if (m >= 0) return m < n_in ? in_row[m] : make_float2(0.f, 0.f);
-    return m >= -(HALF - 1) ? hist_row[HALF - 1 + m] : make_float2(0.f, 0.f);
+    return m >= -HIST ? hist_row[HIST + m] : make_float2(0.f, 0.f);
 }
 
 
+template <int HK, int R>
 __global__ void __launch_bounds__(THREADS, 1) spiir_up2_tc_kernel(const UpTcArgs a, const __grid_constant__ CUtensorMap in_map)
 {
+    using G = Geo<HK, R>;
+
     extern __shared__ __align__(1024) unsigned char sm[];
     const uint32_t sbase = s32(sm);
-    const uint32_t bar0 = sbase + OFF_BAR;
+    const uint32_t bar0 = sbase + G::OFF_BAR;
     auto full = [&](int i) { return bar0 + 8u * (uint32_t)i; };
-    auto empty = [&](int i) { return bar0 + 8u * (uint32_t)(RING_CH + i); };
-    auto tfull = [&](int i) { return bar0 + 8u * (uint32_t)(2 * RING_CH + i); };
-    auto tempty = [&](int i) { return bar0 + 8u * (uint32_t)(2 * RING_CH + 2 + i); };
-    auto sfull = [&](int i) { return bar0 + 8u * (uint32_t)(2 * RING_CH + 4 + i); };
-    auto sempty = [&](int i) { return bar0 + 8u * (uint32_t)(2 * RING_CH + 4 + STG_SLOTS + i); };
-    uint32_t* tptr = reinterpret_cast<uint32_t*>(sm + OFF_TPTR);
+    auto empty = [&](int i) { return bar0 + 8u * (uint32_t)(G::RING_CH + i); };
+    auto tfull = [&](int i) { return bar0 + 8u * (uint32_t)(2 * G::RING_CH + i); };
+    auto tempty = [&](int i) { return bar0 + 8u * (uint32_t)(2 * G::RING_CH + 2 + i); };
+    auto sfull = [&](int i) { return bar0 + 8u * (uint32_t)(2 * G::RING_CH + 4 + i); };
+    auto sempty = [&](int i) { return bar0 + 8u * (uint32_t)(2 * G::RING_CH + 4 + STG_SLOTS + i); };
+    uint32_t* tptr = reinterpret_cast<uint32_t*>(sm + G::OFF_TPTR);
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int ph = phase_read(a.phase);
     const float2* hcur = a.hbuf[ph];
@@ -239,7 +257,7 @@ __global__ void __launch_bounds__(THREADS, 1) spiir_up2_tc_kernel(const UpTcArgs
 
     // ---- one-time setup: barriers, tensor memory, the Toeplitz operand into TMEM --------------------------
     if (tid == 0) {
-        for (int i = 0; i < RING_CH; ++i) { bar_init(full(i), LOADER_WARPS); bar_init(empty(i), 1); }
+        for (int i = 0; i < G::RING_CH; ++i) { bar_init(full(i), LOADER_WARPS); bar_init(empty(i), 1); }
         for (int i = 0; i < 2; ++i) { bar_init(tfull(i), 1); bar_init(tempty(i), EPI_WARPS); }
         for (int i = 0; i < STG_SLOTS; ++i) { bar_init(sfull(i), 1); bar_init(sempty(i), LOADER_WARPS); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -255,10 +273,10 @@ __global__ void __launch_bounds__(THREADS, 1) spiir_up2_tc_kernel(const UpTcArgs
     if (warp >= LOADER_WARPS && warp < LOADER_WARPS + 4) {             // lane t of TMEM = output t of a tile
         const int t = (warp & 3) * 32 + lane;
         const uint32_t lane_addr = tmem + ((uint32_t)((warp & 3) * 32) << 16);
-        // T[t = 2m'+p][k] = 2 h[2 (96 + m' - k) + p] for 1 <= k - m' <= 96, split into a TF32-exact high part and the
-        // float32 remainder, computed from the 192 taps (L1-resident) straight into this thread's TMEM lane
+        // T[t = 2m'+p][k] = 2 h[2 (HK + m' - k) + p] for HK - R < k - m' <= HK, split into a TF32-exact high part and the
+        // float32 remainder, computed from the taps (L1-resident) straight into this thread's TMEM lane
         const int mp = t >> 1, pp = t & 1;
-        for (int c0 = 0; c0 < KWIN; c0 += 32) {
+        for (int c0 = 0; c0 < G::KWIN; c0 += 32) {
             uint32_t vh[32], vlb[16], vb[16];
 #pragma unroll
             for (int i = 0; i < 16; ++i) {
@@ -266,7 +284,7 @@ __global__ void __launch_bounds__(THREADS, 1) spiir_up2_tc_kernel(const UpTcArgs
 #pragma unroll
                 for (int e = 0; e < 2; ++e) {
                     const int dk = c0 + 2 * i + e - mp;
-                    v[e] = (dk >= 1 && dk <= HALF) ? 2.f * __ldg(a.taps + 2 * (HALF - dk) + pp) : 0.f;
+                    v[e] = (dk <= HK && dk > HK - R) ? 2.f * __ldg(a.taps + 2 * (HK - dk) + pp) : 0.f;
                     const float h = tf32_hi(v[e]);
                     vh[2 * i + e] = __float_as_uint(h);
                     l[e] = v[e] - h;
@@ -274,9 +292,9 @@ __global__ void __launch_bounds__(THREADS, 1) spiir_up2_tc_kernel(const UpTcArgs
                 vlb[i] = bf16x2(l[0], l[1]);
                 vb[i] = bf16x2(v[0], v[1]);
             }
-            tmem_st32(lane_addr + COL_THI + (uint32_t)c0, vh);
-            tmem_st16(lane_addr + COL_TLB + (uint32_t)(c0 >> 1), vlb);
-            tmem_st16(lane_addr + COL_TB + (uint32_t)(c0 >> 1), vb);
+            tmem_st32(lane_addr + G::COL_THI + (uint32_t)c0, vh);
+            tmem_st16(lane_addr + G::COL_TLB + (uint32_t)(c0 >> 1), vlb);
+            tmem_st16(lane_addr + G::COL_TB + (uint32_t)(c0 >> 1), vb);
         }
         asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
     }
@@ -292,7 +310,7 @@ __global__ void __launch_bounds__(THREADS, 1) spiir_up2_tc_kernel(const UpTcArgs
         const int J = min(a.seg_tiles, a.tiles_per_row - tile0);
         const int ms = tile0 * TIN;
         const int row0 = strip * ROWS;
-        const int nch = WIN_CH - 2 + 2 * J;                            // chunks of this unit: 3 of halo + 2 per tile
+        const int nch = G::WIN_CH - 2 + 2 * J;                            // chunks of this unit: 3 of halo + 2 per tile
 
         // A chunk that lies inside the block with 16-byte aligned rows is STAGED: one thread fetches its raw samples with
         // two TMA tile copies (ROWS rows x 16 samples each, through the tensor map of `in`) into a ring of STG_SLOTS slots,
@@ -301,7 +319,7 @@ __global__ void __launch_bounds__(THREADS, 1) spiir_up2_tc_kernel(const UpTcArgs
         // for the newest; one bulk copy per row was no better: the TMA unit took ~70 cycles per 256-byte request.)
         // Other chunks (history in front of the block, ragged end, unaligned rows) are read element by element.
         auto staged = [&](int ci) {
-            const int mc = ms - HALF + ci * CHS;
+            const int mc = ms - HK + ci * CHS;
             return a.in16 && mc >= 0 && mc + CHS <= a.n_in;
         };
         if (warp < LOADER_WARPS) {
@@ -310,24 +328,24 @@ __global__ void __launch_bounds__(THREADS, 1) spiir_up2_tc_kernel(const UpTcArgs
             // (consecutive lanes = consecutive rows; the 128-byte swizzle puts piece j of row r at j ^ (r mod 8):
             // conflict-free) and, after the split, four 16-byte stores (re / im, high / low; consecutive lanes =
             // consecutive 16-byte slots of one unit: conflict-free). =====
-            const int hfirst = a.n_in - (HALF - 1);                     // first block sample that is part of the next history
+            const int hfirst = a.n_in - G::HIST;                     // first block sample that is part of the next history
             // Carried history of this strip's rows = the last 95 samples of (history ++ block).  A block of at least 95 samples
             // supplies all of them, and they pass through the loaders' registers anyway (written below); shorter blocks
             // take this explicit copy.
             if (seg == 0 && hfirst < 0) {
-                for (int i = tid; i < ROWS * (HALF - 1); i += LOADERS) {
-                    const int rr = i / (HALF - 1), k = i % (HALF - 1), rw = row0 + rr;
+                for (int i = tid; i < ROWS * G::HIST; i += LOADERS) {
+                    const int rr = i / G::HIST, k = i % G::HIST, rw = row0 + rr;
                     if (rw < a.rows) {
-                        const int g = a.n_in - (HALF - 1) + k;
-                        hnext[(size_t)rw * (HALF - 1) + k] =
-                            g >= 0 ? a.in[(size_t)rw * a.n_in + g] : hcur[(size_t)rw * (HALF - 1) + a.n_in + k];
+                        const int g = a.n_in - G::HIST + k;
+                        hnext[(size_t)rw * G::HIST + k] =
+                            g >= 0 ? a.in[(size_t)rw * a.n_in + g] : hcur[(size_t)rw * G::HIST + a.n_in + k];
                     }
                 }
             }
             int sc = sbase_ch;
             for (int ci = 0; ci < nch; ++ci) {
-                const int c = cbase + ci, slot = c % RING_CH, fill = c / RING_CH;
-                const int mc = ms - HALF + ci * CHS;                    // first sample of the chunk
+                const int c = cbase + ci, slot = c % G::RING_CH, fill = c / G::RING_CH;
+                const int mc = ms - HK + ci * CHS;                    // first sample of the chunk
                 const bool stg = staged(ci);
                 const int ss = sc % STG_SLOTS;
                 constexpr int ITEMS = 2;                                // two units of 4 samples: 8 consecutive samples of row r
@@ -338,7 +356,7 @@ __global__ void __launch_bounds__(THREADS, 1) spiir_up2_tc_kernel(const UpTcArgs
 #pragma unroll
                     for (int k = 0; k < ITEMS; ++k) {
                         const int u = 2 * up + k;
-                        const uint32_t src = sbase + OFF_STG + (uint32_t)(ss * STG_BYTES + (u >> 2) * STG_HALF + r * 128);
+                        const uint32_t src = sbase + G::OFF_STG + (uint32_t)(ss * STG_BYTES + (u >> 2) * STG_HALF + r * 128);
                         const int j = 2 * (u & 3), x = r & 7;
                         v[k][0] = lds128(src + (uint32_t)((j ^ x) << 4));
                         v[k][1] = lds128(src + (uint32_t)(((j + 1) ^ x) << 4));
@@ -356,27 +374,27 @@ __global__ void __launch_bounds__(THREADS, 1) spiir_up2_tc_kernel(const UpTcArgs
                         for (int e = 0; e < 4; ++e) q[e] = make_float2(0.f, 0.f);
                         if (row < a.rows) {
                             const float2* in_row = a.in + (size_t)row * a.n_in;
-                            const float2* hist_row = hcur + (size_t)row * (HALF - 1);
+                            const float2* hist_row = hcur + (size_t)row * G::HIST;
 #pragma unroll
-                            for (int e = 0; e < 4; ++e) q[e] = sample_at(in_row, hist_row, m + e, a.n_in);
+                            for (int e = 0; e < 4; ++e) q[e] = sample_at<G::HIST>(in_row, hist_row, m + e, a.n_in);
                         }
                         v[k][0] = make_float4(q[0].x, q[0].y, q[1].x, q[1].y);
                         v[k][1] = make_float4(q[2].x, q[2].y, q[3].x, q[3].y);
                     }
                 }
                 // the next history = the block's last 95 samples: written by the unit that owns them (not from a halo)
-                if (ci >= HALO_CH && hfirst >= 0 && mc + CHS > hfirst) {
+                if (ci >= G::HALO_CH && hfirst >= 0 && mc + CHS > hfirst) {
 #pragma unroll
                     for (int k = 0; k < ITEMS; ++k) {
                         const int u = 2 * up + k;
                         const int row = row0 + r, g = mc + 4 * u - hfirst;
                         if (row < a.rows) {
-                            float2* hrow = hnext + (size_t)row * (HALF - 1);
+                            float2* hrow = hnext + (size_t)row * G::HIST;
                             const float2 q[4] = {make_float2(v[k][0].x, v[k][0].y), make_float2(v[k][0].z, v[k][0].w),
                                                  make_float2(v[k][1].x, v[k][1].y), make_float2(v[k][1].z, v[k][1].w)};
 #pragma unroll
                             for (int e = 0; e < 4; ++e)
-                                if (g + e >= 0 && g + e < HALF - 1 && mc + 4 * u + e < a.n_in) hrow[g + e] = q[e];
+                                if (g + e >= 0 && g + e < G::HIST && mc + 4 * u + e < a.n_in) hrow[g + e] = q[e];
                         }
                     }
                 }
@@ -399,10 +417,10 @@ __global__ void __launch_bounds__(THREADS, 1) spiir_up2_tc_kernel(const UpTcArgs
                 }
                 {
                     const uint32_t addr = sbase + (uint32_t)(slot * (CHU / 2) + up) * UNIT_BYTES + (uint32_t)r * 16;
-                    sts128u(addr + OFF_XB, bre[0], bre[1], bre[2], bre[3]);
-                    sts128u(addr + OFF_XB + ROWS * 16, bim[0], bim[1], bim[2], bim[3]);
-                    sts128u(addr + OFF_XLB, lre[0], lre[1], lre[2], lre[3]);
-                    sts128u(addr + OFF_XLB + ROWS * 16, lim[0], lim[1], lim[2], lim[3]);
+                    sts128u(addr + G::OFF_XB, bre[0], bre[1], bre[2], bre[3]);
+                    sts128u(addr + G::OFF_XB + ROWS * 16, bim[0], bim[1], bim[2], bim[3]);
+                    sts128u(addr + G::OFF_XLB, lre[0], lre[1], lre[2], lre[3]);
+                    sts128u(addr + G::OFF_XLB + ROWS * 16, lim[0], lim[1], lim[2], lim[3]);
                 }
                 asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
                 __syncwarp();
@@ -419,8 +437,8 @@ __global__ void __launch_bounds__(THREADS, 1) spiir_up2_tc_kernel(const UpTcArgs
                     const int ss = sc % STG_SLOTS, f = sc / STG_SLOTS;
                     if (f > 0) bar_wait(sempty(ss), (uint32_t)((f - 1) & 1));
                     bar_expect_tx(sfull(ss), (uint32_t)STG_BYTES);
-                    const int c0 = 2 * (ms - HALF + ci * CHS);          // float index of the chunk's first sample
-                    const uint32_t dst = sbase + OFF_STG + (uint32_t)(ss * STG_BYTES);
+                    const int c0 = 2 * (ms - HK + ci * CHS);          // float index of the chunk's first sample
+                    const uint32_t dst = sbase + G::OFF_STG + (uint32_t)(ss * STG_BYTES);
                     tma_g2s_2d(dst, &in_map, c0, row0, sfull(ss));
                     tma_g2s_2d(dst + STG_HALF, &in_map, c0 + 32, row0, sfull(ss));
                     ++sc;
@@ -434,35 +452,35 @@ __global__ void __launch_bounds__(THREADS, 1) spiir_up2_tc_kernel(const UpTcArgs
                 const uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(NR >> 3) << 17) | ((uint32_t)(MOUT >> 4) << 24);
                 const uint32_t idesc_bf = (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(NR >> 3) << 17) | ((uint32_t)(MOUT >> 4) << 24);
                 for (int j = 0; j < J; ++j) {
-                    const int cn = cbase + 2 * j + WIN_CH - 1;          // newest chunk of this tile's window
-                    bar_wait(full(cn % RING_CH), (uint32_t)((cn / RING_CH) & 1));
-                    const int t = tbase + j, buf = t % NBUF, use = t / NBUF;
+                    const int cn = cbase + 2 * j + G::WIN_CH - 1;          // newest chunk of this tile's window
+                    bar_wait(full(cn % G::RING_CH), (uint32_t)((cn / G::RING_CH) & 1));
+                    const int t = tbase + j, buf = t % G::NBUF, use = t / G::NBUF;
                     if (use > 0) bar_wait(tempty(buf), (uint32_t)((use - 1) & 1));   // this buffer's previous tile has been drained
-                    const uint32_t d = tmem + COL_D + (uint32_t)(buf * NR);
+                    const uint32_t d = tmem + G::COL_D + (uint32_t)(buf * NR);
                     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-                    const int wu0 = ((cbase + 2 * j) % RING_CH) * CHU;  // ring unit of the window's first unit
+                    const int wu0 = ((cbase + 2 * j) % G::RING_CH) * CHU;  // ring unit of the window's first unit
                     // T_hi X_hi in TF32 (20 instructions of K = 8), then the two correction terms bf16(T_lo) bf16(X) and
                     // bf16(T) bf16(X_lo) with bf16 operands (10 + 10 instructions of K = 16) into the same accumulator
 #pragma unroll 2
-                    for (int ks = 0; ks < KSTEPS; ++ks) {
+                    for (int ks = 0; ks < G::KSTEPS; ++ks) {
                         int ru = wu0 + 2 * ks;
-                        if (ru >= RING_UNITS) ru -= RING_UNITS;
-                        umma_tf32_ts(d, tmem + COL_THI + (uint32_t)(8 * ks), smem_desc(sbase + (uint32_t)ru * UNIT_BYTES, UNIT_BYTES, 128),
+                        if (ru >= G::RING_UNITS) ru -= G::RING_UNITS;
+                        umma_tf32_ts(d, tmem + G::COL_THI + (uint32_t)(8 * ks), smem_desc(sbase + (uint32_t)ru * UNIT_BYTES, UNIT_BYTES, 128),
                                      idesc, ks > 0 ? 1u : 0u);
                     }
 #pragma unroll 2
-                    for (int ks = 0; ks < KSTEPS / 2; ++ks) {
+                    for (int ks = 0; ks < G::KSTEPS / 2; ++ks) {
                         int ru = (wu0 >> 1) + 2 * ks;                   // units of 8 samples
-                        if (ru >= RING_UNITS / 2) ru -= RING_UNITS / 2;
+                        if (ru >= G::RING_UNITS / 2) ru -= G::RING_UNITS / 2;
                         const uint32_t xb = sbase + (uint32_t)ru * UNIT_BYTES;
-                        umma_bf16_ts(d, tmem + COL_TLB + (uint32_t)(8 * ks), smem_desc(xb + OFF_XB, UNIT_BYTES, 128), idesc_bf, 1u);
-                        umma_bf16_ts(d, tmem + COL_TB + (uint32_t)(8 * ks), smem_desc(xb + OFF_XLB, UNIT_BYTES, 128), idesc_bf, 1u);
+                        umma_bf16_ts(d, tmem + G::COL_TLB + (uint32_t)(8 * ks), smem_desc(xb + G::OFF_XB, UNIT_BYTES, 128), idesc_bf, 1u);
+                        umma_bf16_ts(d, tmem + G::COL_TB + (uint32_t)(8 * ks), smem_desc(xb + G::OFF_XLB, UNIT_BYTES, 128), idesc_bf, 1u);
                     }
-                    umma_commit(empty((cbase + 2 * j) % RING_CH));     // the window's two oldest chunks are free once these MMAs are done
-                    umma_commit(empty((cbase + 2 * j + 1) % RING_CH));
+                    umma_commit(empty((cbase + 2 * j) % G::RING_CH));     // the window's two oldest chunks are free once these MMAs are done
+                    umma_commit(empty((cbase + 2 * j + 1) % G::RING_CH));
                     umma_commit(tfull(buf));
                 }
-                for (int i = 0; i < HALO_CH; ++i) umma_commit(empty((cbase + 2 * J + i) % RING_CH));
+                for (int i = 0; i < G::HALO_CH; ++i) umma_commit(empty((cbase + 2 * J + i) % G::RING_CH));
             }
             __syncwarp();
         } else {
@@ -473,11 +491,11 @@ __global__ void __launch_bounds__(THREADS, 1) spiir_up2_tc_kernel(const UpTcArgs
             const int ew = warp & 3;
             const int tl = ew * 32 + lane;                              // output index within the tile
             for (int j = 0; j < J; ++j) {
-                const int t = tbase + j, buf = t % NBUF, use = t / NBUF;
+                const int t = tbase + j, buf = t % G::NBUF, use = t / G::NBUF;
                 const int m0 = ms + j * TIN;
                 const bool tok = tl < 2 * min(TIN, a.n_in - m0);
                 float2* obase = a.out + (size_t)row0 * 2 * a.n_in + 2 * m0 + tl;
-                const uint32_t taddr = tmem + ((uint32_t)(ew * 32) << 16) + COL_D + (uint32_t)(buf * NR);
+                const uint32_t taddr = tmem + ((uint32_t)(ew * 32) << 16) + G::COL_D + (uint32_t)(buf * NR);
                 bar_wait(tfull(buf), (uint32_t)(use & 1));
                 asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
                 // drain in two halves (ROWS registers each); the buffer is released right after the second drain
