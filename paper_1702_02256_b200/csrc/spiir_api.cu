@@ -132,7 +132,14 @@ static filter_kernel_t pick_kernel(int F, int LPT, int NP, bool noz)
         case 1: return pick_small<1>(F, noz);
         case 2: return pick_small<2>(F, noz);
         case 4: return pick_small<4>(F, noz);
-        case 8: return pick_small<8>(F, noz);
+        case 8:
+            switch (F) {
+                case 5: return pick_noz<5, 8>(noz);
+                case 6: return pick_noz<6, 8>(noz);
+                case 7: return pick_noz<7, 8>(noz);
+                case 8: return pick_noz<8, 8>(noz);
+            }
+            return pick_small<8>(F, noz);
         case 16:
             switch (F) {
                 case 2: return pick_noz<2, 16>(noz);

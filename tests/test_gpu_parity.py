@@ -83,13 +83,14 @@ def test_config1_full_size_sampled(sp, oracle_mod):
 
 
 def test_half_warp_per_template_mapping(sp, oracle_mod):
-    """Banks of 32..128 filters with >= 2368 templates put two templates in a warp (16 lanes each)."""
-    for L in (40, 128):
+    """Banks with >= 2368 templates: 32..64 filters put four templates in a warp (8 lanes each), 65..128 two (16 lanes)."""
+    for L in (32, 40, 64, 72, 128):
         w = _inputs().config(1, n_templates=2400, n_filters=L)
         b = w.banks[0]
         plan = sp.Plan(b.a1, b.b0, b.delays % 300, b.rate_hz, max_block=256)
         info = plan.launch_info(256)
-        assert info["lanes_per_template"] == 16 and info["F"] == (L + 15) // 16
+        lpt = 8 if L <= 64 else 16
+        assert info["lanes_per_template"] == lpt and info["F"] == (L + lpt - 1) // lpt
         rng = np.random.default_rng(L)
         xs = [rng.standard_normal((1, n)).astype(np.float32) for n in (256, 37, 160)]
         z = stream_gpu_plan(plan, xs)

@@ -150,9 +150,16 @@ def test_chunking_follows_the_cost_model(sp):
 
 
 def test_lane_mapping_many_templates(sp):
-    # 32..128 filters and at least 16 x 148 templates: two templates per warp, 16 lanes each
+    # at least 16 x 148 templates: 32..64 filters take a quarter warp per template (four templates per warp), 65..128
+    # half a warp (two templates per warp)
     g = sp.spiir_host_geometry(4096, 64, 1, 100, 1024)
-    assert (g["F"], g["lanes_per_template"]) == (4, 16)
+    assert (g["F"], g["lanes_per_template"]) == (8, 8)
+    g = sp.spiir_host_geometry(4096, 32, 1, 100, 1024)
+    assert (g["F"], g["lanes_per_template"]) == (4, 8)
+    g = sp.spiir_host_geometry(4096, 65, 1, 100, 1024)
+    assert (g["F"], g["lanes_per_template"]) == (5, 16)
+    g = sp.spiir_host_geometry(4096, 128, 1, 100, 1024)
+    assert (g["F"], g["lanes_per_template"]) == (8, 16)
     g = sp.spiir_host_geometry(4096, 129, 1, 100, 1024)
     assert (g["F"], g["lanes_per_template"]) == (5, 32)
     g = sp.spiir_host_geometry(2367, 64, 1, 100, 1024)
