@@ -416,7 +416,10 @@ struct DownArgs {
     int nseg;
 };
 
-template <int N>
+// R outputs per thread: 6 for 192 and 384 taps, 10 for 32.  The fully unrolled body is R x N FFMAs; at 384 taps and
+// R = 10 (61 KB of code) the kernel ran at the speed of its instruction-cache misses (3.65 ms for 16384 x 4096 -> 2048
+// against 0.65 ms at R = 6).  R = 4 and 8 put the lanes' 16-byte loads 2 or 4 chunks apart: bank conflicts.
+template <int N, int R = kDownR>
 __global__ void __launch_bounds__(128, 8) spiir_down2_fir_kernel(const DownArgs a, const __grid_constant__ DownTaps<N> taps)
 {
     constexpr int H = N - 1;
@@ -425,23 +428,34 @@ __global__ void __launch_bounds__(128, 8) spiir_down2_fir_kernel(const DownArgs 
     const int n_out = a.n_in >> 1;
     const int m_base = seg_idx * a.seg;
     const int seg_len = min(a.seg, n_out - m_base);
-    const int w_len = (2 * a.seg + H + 2 * kDownR + 7) & ~3;           // staged inputs incl. over-read pad
+    const int w_len = (2 * a.seg + H + 2 * R + 7) & ~3;                // staged inputs incl. over-read pad
     float* w = smd;
     float* out_s = smd + w_len;
     const int ph = phase_read(a.phase);
     const float* in = a.in + (size_t)row * a.n_in;
     const float* hist = a.hbuf[ph] + (size_t)row * H;
-    for (int i = threadIdx.x; i < w_len; i += blockDim.x) {
-        const int g = 2 * m_base - H + i;
-        float v = 0.f;
-        if (i < 2 * seg_len + H) {
-            if (g >= 0) v = in[g];
-            else if (H + g >= 0) v = hist[H + g];
+    // eight independent loads in flight per thread (a rolled loop keeps one: 21 DRAM round trips in a row per CTA;
+    // 192 taps: 472 -> 362 us)
+    for (int i0 = threadIdx.x; i0 < w_len; i0 += 8 * blockDim.x) {
+        float v[8];
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+            const int i = i0 + k * blockDim.x;
+            const int g = 2 * m_base - H + i;
+            v[k] = 0.f;
+            if (i < 2 * seg_len + H) {
+                if (g >= 0) v[k] = in[g];
+                else if (H + g >= 0) v[k] = hist[H + g];
+            }
         }
-        w[i] = v;
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+            const int i = i0 + k * blockDim.x;
+            if (i < w_len) w[i] = v[k];
+        }
     }
     __syncthreads();
-    down2_units<N>(w, seg_len, out_s, taps, threadIdx.x, blockDim.x);
+    down2_units<N, R>(w, seg_len, out_s, taps, threadIdx.x, blockDim.x);
     __syncthreads();
     float* o = a.out + (size_t)row * n_out + m_base;
     for (int i = threadIdx.x; i < seg_len; i += blockDim.x) o[i] = out_s[i];
