@@ -269,11 +269,20 @@ spiir_status spiir_resample_up(spiir_resamp_t* r, const spiir_c64* in, int n_in,
         t.rows = r->rows; t.n_in = n_in; t.accumulate = accumulate;
         t.tiles_per_row = (n_in + tc::TIN - 1) / tc::TIN;
         t.nstrips = (r->rows + tc::ROWS - 1) / tc::ROWS;
-        const int want = 6 * r->dev.n_sm;                    // units per launch for an even tail
-        int nsegs = t.nstrips >= want ? 1 : std::min((t.tiles_per_row + 3) / 4, (want + t.nstrips - 1) / t.nstrips);
-        nsegs = std::max(1, nsegs);
-        t.seg_tiles = (t.tiles_per_row + nsegs - 1) / nsegs;
-        t.nsegs = (t.tiles_per_row + t.seg_tiles - 1) / t.seg_tiles;
+        // Time segments per strip: a unit (strip, segment) costs its tiles plus 1.5 tile-times of halo, the persistent CTAs
+        // take the units round-robin; the segment length with the fewest tile-times on the busiest CTA wins (the shortest
+        // on a tie: measured faster, 248 against 261 us on 16384 x 2048).
+        {
+            double best = 1e30;
+            t.seg_tiles = t.tiles_per_row; t.nsegs = 1;
+            for (int st_ = 1; st_ <= t.tiles_per_row; ++st_) {
+                const int ns = (t.tiles_per_row + st_ - 1) / st_;
+                const long units = (long)t.nstrips * ns;
+                const long rounds = (units + r->dev.n_sm - 1) / r->dev.n_sm;
+                const double cost = (double)rounds * (st_ + 1.5);
+                if (cost < best * 0.999) { best = cost; t.seg_tiles = st_; t.nsegs = ns; }
+            }
+        }
         t.in16 = ((reinterpret_cast<uintptr_t>(in) & 15u) == 0 && (n_in & 1) == 0) ? 1 : 0;
         CUtensorMap in_map;
         memset(&in_map, 0, sizeof in_map);
