@@ -270,13 +270,15 @@ __global__ void __launch_bounds__(THREADS, 1) spiir_up2_tc_kernel(const UpTcArgs
     __syncthreads();
     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
     const uint32_t tmem = *tptr;
-    if (warp >= LOADER_WARPS && warp < LOADER_WARPS + 4) {             // lane t of TMEM = output t of a tile
+    {   // lane t of TMEM = output t of a tile.  A warp reaches the TMEM lanes 32 (warp mod 4) .. + 31: the twelve warps share
+        // the work as three per lane quarter, each taking every third block of 32 columns (one warp per quarter took 6 us)
         const int t = (warp & 3) * 32 + lane;
         const uint32_t lane_addr = tmem + ((uint32_t)((warp & 3) * 32) << 16);
         // T[t = 2m'+p][k] = 2 h[2 (HK + m' - k) + p] for HK - R < k - m' <= HK, split into a TF32-exact high part and the
         // float32 remainder, computed from the taps (L1-resident) straight into this thread's TMEM lane
         const int mp = t >> 1, pp = t & 1;
-        for (int c0 = 0; c0 < G::KWIN; c0 += 32) {
+        static_assert(THREADS == 384, "three warps per TMEM lane quarter");
+        for (int c0 = (warp >> 2) * 32; c0 < G::KWIN; c0 += 3 * 32) {
             uint32_t vh[32], vlb[16], vb[16];
 #pragma unroll
             for (int i = 0; i < 16; ++i) {
