@@ -29,6 +29,9 @@ __device__ __forceinline__ bool last_cta_arrives(int* w, int total_ctas)
 // parity of the number of finished launches, w[1] / kPhaseUnit.  A CTA that reads the word while its own launch is
 // under way sees a partial sum below the next multiple, i.e. still the phase the launch started with.  The shares of one
 // launch add up to kPhaseUnit whatever its grid, so calls with different block lengths can follow one another.
+// ONE thread per CTA reads the word and then adds (same address: program order holds) and hands the value to the others
+// through shared memory; threads that each read the word themselves may read it after the CTA's own share and the last
+// share of the launch have landed.
 constexpr int kPhaseUnit = 1 << 16;                 // grids of up to 65536 CTAs; 2^32 is a multiple, so wrap-around is harmless
 __device__ __forceinline__ int phase_parity(const int* w)
 {

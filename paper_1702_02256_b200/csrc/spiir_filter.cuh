@@ -383,13 +383,20 @@ __device__ __forceinline__ void filter_body(const FilterArgs& a, const int bx, c
     const int s = by / a.NC, c = by % a.NC;
     const int tc0 = c * a.C;                                            // chunk range [tc0, tc1)
     const int tc1 = min(a.n, tc0 + a.C);
-    const int ph = phase_parity(a.phase);
-    if (a.carry && threadIdx.x == 0) phase_arrive(a.phase, by * gdx + bx, gdx * gdy);   // no one waits for this
+    // ONE thread reads the phase word and then adds the CTA's share (same address, program order); everybody else takes
+    // the value from shared memory.  A thread that read the word itself could do so after the launch's last share had
+    // landed -- nothing orders the warps of a CTA between the read and the add -- and see the NEXT phase.
+    int* sph = reinterpret_cast<int*>(bar + 1);                          // the 8 bytes behind the mbarrier are free
+    uint32_t parity = 0;
+    if (threadIdx.x == 0) {
+        mbar_init(bar, 1);
+        *sph = phase_parity(a.phase);
+        if (a.carry) phase_arrive(a.phase, by * gdx + bx, gdx * gdy);    // no one waits for this
+    }
+    __syncthreads();
+    const int ph = *sph;
     const float* hist_s = a.hbuf[ph] + (size_t)s * a.Dpad;
     const float* x_s = a.x + (size_t)s * a.n;
-    uint32_t parity = 0;
-    if (threadIdx.x == 0) mbar_init(bar, 1);
-    __syncthreads();
     const int ntiles = (tc1 - tc0 + a.NT - 1) / a.NT;
     // single-tile case: the window is staged once, AFTER the first group's coefficient / state loads have been
     // issued (below), so that their DRAM round trip overlaps the TMA copy and the shifted copies
@@ -547,13 +554,17 @@ __global__ void __launch_bounds__(kScanMaxWarps * 32) spiir_filter_scan_kernel(c
         Y[f] = (c == 0) ? st[(size_t)f * 32] : make_float2(0.f, 0.f);
         if (a.apow) aC[f] = a.apow[lbase + (size_t)f * 32];           // a1^C from the plan's table (same chunk length)
     }
-    const int ph = phase_parity(a.phase);
-    if (a.carry && threadIdx.x == 0) phase_arrive(a.phase, blockIdx.y * gridDim.x + blockIdx.x, gridDim.x * gridDim.y);
+    int* sph = reinterpret_cast<int*>(bar + 1);                          // one reader of the phase word per CTA: see filter_body
+    uint32_t parity = 0;
+    if (threadIdx.x == 0) {
+        mbar_init(bar, 1);
+        *sph = phase_parity(a.phase);
+        if (a.carry) phase_arrive(a.phase, blockIdx.y * gridDim.x + blockIdx.x, gridDim.x * gridDim.y);
+    }
+    __syncthreads();
+    const int ph = *sph;
     const float* hist_s = a.hbuf[ph] + (size_t)s * a.Dpad;
     const float* x_s = a.x + (size_t)s * a.n;
-    uint32_t parity = 0;
-    if (threadIdx.x == 0) mbar_init(bar, 1);
-    __syncthreads();
 #pragma unroll
     for (int f = 0; f < F; ++f) {
         const int d = dl[f];

@@ -141,6 +141,30 @@ def test_in_cta_time_scan(sp, oracle_mod, T, L, S, chunks, blocks):
     assert_parity(plain, ref, "plain")
 
 
+def test_phase_word_has_one_reader_per_cta(sp, oracle_mod):
+    """Regression (found by a randomised parity run): every thread used to read the ping-pong phase word itself, so a slow
+    warp of a late CTA could read it after the launch's last share had landed and take the NEXT phase -- the wrong history
+    buffer for its templates, about one fresh plan in four with this shape (450 CTAs of 5 warps, three streams).  Twelve
+    fresh plans, one block each, every output compared."""
+    import torch
+    rng = np.random.default_rng(5)
+    T, L, S, n = 600, 24, 3, 1130
+    mag, arg = rng.uniform(0.5, 0.9999, (T, L)), rng.uniform(0, 2 * np.pi, (T, L))
+    a1 = (mag * np.exp(1j * arg)).astype(np.complex64)
+    b0 = (1e-3 * (rng.standard_normal((T, L)) + 1j * rng.standard_normal((T, L)))).astype(np.complex64)
+    d = rng.integers(0, 101, (T, L)).astype(np.int32)
+    x = rng.standard_normal((S, n)).astype(np.float32)
+    ref = oracle_mod.FilterOracle(a1, b0, d, S).filter(x)
+    xd = torch.from_numpy(x).cuda()
+    for trial in range(12):
+        plan = sp.Plan(a1, b0, d, 4096, n_streams=S, max_block=2048)
+        z = plan.filter(xd).cpu().numpy()
+        hist = plan.get_state()[1].cpu().numpy()
+        plan.close()
+        assert_parity(z, ref, f"fresh plan {trial}")
+        np.testing.assert_array_equal(hist, x[:, -hist.shape[1]:])
+
+
 def test_config2_bulk_call_sampled(sp, oracle_mod):
     """configs[2] as ONE call of 64 x 256 = 16384 samples (the bulk shape bench.py times), L = 1 and 4: full bank on the
     GPU, the oracle on templates spread over every CTA (first and last included)."""
