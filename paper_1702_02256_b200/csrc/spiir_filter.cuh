@@ -386,16 +386,19 @@ __device__ __forceinline__ void filter_body(const FilterArgs& a, const int bx, c
     // ONE thread reads the phase word and then adds the CTA's share (same address, program order); everybody else takes
     // the value from shared memory.  A thread that read the word itself could do so after the launch's last share had
     // landed -- nothing orders the warps of a CTA between the read and the add -- and see the NEXT phase.
+    // The value is handed over only in front of the first window (below): its DRAM round trip overlaps the first
+    // group's coefficient / state loads.
     int* sph = reinterpret_cast<int*>(bar + 1);                          // the 8 bytes behind the mbarrier are free
     uint32_t parity = 0;
+    int ph = 0;
     if (threadIdx.x == 0) {
         mbar_init(bar, 1);
-        *sph = phase_parity(a.phase);
+        ph = phase_parity(a.phase);
         if (a.carry) phase_arrive(a.phase, by * gdx + bx, gdx * gdy);    // no one waits for this
     }
     __syncthreads();
-    const int ph = *sph;
-    const float* hist_s = a.hbuf[ph] + (size_t)s * a.Dpad;
+    bool ph_known = false;
+    const float* hist_s = nullptr;
     const float* x_s = a.x + (size_t)s * a.n;
     const int ntiles = (tc1 - tc0 + a.NT - 1) / a.NT;
     // single-tile case: the window is staged once, AFTER the first group's coefficient / state loads have been
@@ -439,6 +442,13 @@ __device__ __forceinline__ void filter_body(const FilterArgs& a, const int bx, c
         oc.tile = red + (size_t)warp * (TPG * kTileRow4);
         oc.active = active; oc.acc = a.accumulate != 0; oc.z16 = a.z16 != 0;
         out_ctx_rows<LPT>(oc, a, g, lane);
+        if (!ph_known) {                                                // first group only (uniform over the CTA)
+            if (threadIdx.x == 0) *sph = ph;
+            __syncthreads();
+            ph = *sph;
+            hist_s = a.hbuf[ph] + (size_t)s * a.Dpad;
+            ph_known = true;
+        }
         if (!staged) { stage_window(win, bar, parity, a, hist_s, x_s, tc0); staged = true; }
 
         for (int tile = 0; tile < ntiles; ++tile) {
@@ -470,6 +480,12 @@ __device__ __forceinline__ void filter_body(const FilterArgs& a, const int bx, c
     // carried history for the next block (reads only hist + x, writes the other buffer: no race with other CTAs).  Every
     // CTA of the stream copies a slice, at the END of its life: by then x and the history are in L2 and the copy is off
     // the critical path (at the top it was a chain of DRAM round trips in front of the coefficient loads).
+    if (!ph_known) {                                                    // a CTA without a group (cannot happen with the host's grids)
+        if (threadIdx.x == 0) *sph = ph;
+        __syncthreads();
+        ph = *sph;
+        hist_s = a.hbuf[ph] + (size_t)s * a.Dpad;
+    }
     if (a.carry) {
         float* hn = a.hbuf[ph ^ 1] + (size_t)s * a.Dpad;
         const int cta = c * gdx + bx, nctas = a.NC * gdx;
