@@ -421,20 +421,23 @@ __device__ __forceinline__ void filter_body(const FilterArgs& a, const int bx, c
         const int t = active ? (a.tmap ? a.tmap[tl] : tl) : 0;          // output row
         float4 cf[F]; float2 Y[F]; int off4[F];
         const size_t lbase = ((size_t)(wactive ? g : 0) * F) * 32 + lane;
+        // All 3 F loads of the lane are issued before any of them is used, from ONE address per array chosen without a
+        // branch.  (With the delay consumed inside the loop and the state behind an if / else, ptxas kept the loop order:
+        // F DRAM round trips in a row, 6 us of the 9.5 us prologue of configs[1].)
+        const float2* ysrc = a.mode == 2 ? a.chunk_st + (((size_t)s * a.NC + c) * a.G * F) * 32 + lbase
+                                         : a.state + (size_t)s * a.sstride + lbase;
+        const bool yload = wactive && (a.mode == 0 || a.mode == 2 || (a.mode == 1 && c == 0));
+        int dl[F];
 #pragma unroll
         for (int f = 0; f < F; ++f) {
             cf[f] = wactive ? a.coef[lbase + (size_t)f * 32] : make_float4(0.f, 0.f, 0.f, 0.f);
-            const int d = wactive ? a.dly[lbase + (size_t)f * 32] : 0;
-            const int sh = (-d) & 3;
-            off4[f] = (sh * a.CS + a.Dpad - d - sh) >> 2;
-            float2 y0 = make_float2(0.f, 0.f);
-            if (wactive) {
-                if (a.mode == 0 || (a.mode == 1 && c == 0))
-                    y0 = a.state[(size_t)s * a.sstride + lbase + (size_t)f * 32];
-                else if (a.mode == 2)
-                    y0 = a.chunk_st[(((size_t)s * a.NC + c) * a.G * F) * 32 + lbase + (size_t)f * 32];
-            }
-            Y[f] = y0;
+            dl[f] = wactive ? a.dly[lbase + (size_t)f * 32] : 0;
+            Y[f] = yload ? ysrc[(size_t)f * 32] : make_float2(0.f, 0.f);
+        }
+#pragma unroll
+        for (int f = 0; f < F; ++f) {
+            const int sh = (-dl[f]) & 3;
+            off4[f] = (sh * a.CS + a.Dpad - dl[f] - sh) >> 2;
         }
         OutCtx<LPT> oc;
         oc.zt = active ? a.z + ((size_t)s * a.T_rows + t) * (size_t)a.n : nullptr;
