@@ -434,11 +434,6 @@ __device__ __forceinline__ void filter_body(const FilterArgs& a, const int bx, c
             dl[f] = wactive ? a.dly[lbase + (size_t)f * 32] : 0;
             Y[f] = yload ? ysrc[(size_t)f * 32] : make_float2(0.f, 0.f);
         }
-#pragma unroll
-        for (int f = 0; f < F; ++f) {
-            const int sh = (-dl[f]) & 3;
-            off4[f] = (sh * a.CS + a.Dpad - dl[f] - sh) >> 2;
-        }
         OutCtx<LPT> oc;
         oc.zt = active ? a.z + ((size_t)s * a.T_rows + t) * (size_t)a.n : nullptr;
         oc.z_s = a.z + (size_t)s * a.T_rows * (size_t)a.n; oc.n = (size_t)a.n;
@@ -453,6 +448,12 @@ __device__ __forceinline__ void filter_body(const FilterArgs& a, const int bx, c
             ph_known = true;
         }
         if (!staged) { stage_window(win, bar, parity, a, hist_s, x_s, tc0); staged = true; }
+        // first use of the loads above: they were in flight while the window was staged
+#pragma unroll
+        for (int f = 0; f < F; ++f) {
+            const int sh = (-dl[f]) & 3;
+            off4[f] = (sh * a.CS + a.Dpad - dl[f] - sh) >> 2;
+        }
 
         for (int tile = 0; tile < ntiles; ++tile) {
             const int t0 = tc0 + tile * a.NT;
